@@ -1,0 +1,621 @@
+// kernels.cuh -- CUDA kernels of libmcb200 (sm_100a).  See DESIGN.md for the decomposition.
+//
+// One sweep = k_trial, then for every chunk of <= 1024 consecutive particles:
+//   k_bulk   rows of the chunk x all columns outside the chunk, current positions   (a2)
+//   k_diag   rows of the chunk x columns of the chunk: base sums at the chunk-start
+//            positions plus, for every j < i, the correction D(i,j) that applies if j's
+//            move is accepted, and the two overlap bit matrices                       (a2/a3)
+//   k_chain  the sequential resolution: decisions in ascending i, D-corrections applied
+//            as accept bits become known (ballot), commit of positions and log       (a3/a4)
+// Because positions are committed in place chunk by chunk, "current positions" seen by
+// k_bulk are x'_j for j before the chunk and x_j after it -- exactly Eq. 2.
+#pragma once
+#include "common.cuh"
+
+namespace mcb {
+
+struct Params {
+    int N, Np, chunk;
+    double2* xy;   // (x, y)  current positions                [Np]
+    double2* zq;   // (z, q)                                   [Np]
+    double* hh;    // d/2                                       [Np]
+    double* lbq;   // l_B q                                     [Np]
+    double2* txy;  // trial (x, y) of this sweep                [Np]
+    double* tz;    // trial z                                   [Np]
+    double* lnu;   // ln(u_acc)                                 [Np]
+    unsigned char* wall;  // kFlagWall if vetoed by the wall    [Np]
+    double* partA; int* ovA;   // [slices][chunk] partial sums / overlap counts of k_bulk
+    double* partD; int* ovD;   // [chunk/32][chunk]              of k_diag
+    double* Dblk;              // [nt(nt+1)/2][32 jj][32 ii] corrections, lower triangle of blocks
+    unsigned* OVold; unsigned* OVnew;  // [chunk][chunk/32] bit jj of word s: trial i overlaps old/new j
+    double* log_dE; unsigned char* log_flags;  // [Np]
+    DevState* st;
+    double R, lB, max_disp;
+    unsigned long long seed;
+};
+
+// ------------------------------------------------------------------------------------------
+// a1: trial generation.  Alg. 1 + old position (G1), D = 2 max_disp (G2),
+// Philox keyed by (seed; particle, sweep, tag) (G9), hard wall (G6).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_trial(Params p) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.Np) return;
+    const double2 xy = p.xy[i];
+    const double2 zq = p.zq[i];
+    if (i >= p.N) {  // ghost padding: never moves
+        p.txy[i] = xy; p.tz[i] = zq.x; p.lnu[i] = 0.0; p.wall[i] = (unsigned char)kFlagWall;
+        return;
+    }
+    const unsigned long long s = p.st->sweep;
+    const uint32_t k0 = (uint32_t)p.seed, k1 = (uint32_t)(p.seed >> 32);
+    uint32_t A[4], B[4];
+    philox4x32_10((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, k0, k1, A);
+    philox4x32_10((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 1u, k0, k1, B);
+    const double ux = uniform_open01(A[0], A[1]);
+    const double uy = uniform_open01(A[2], A[3]);
+    const double uz = uniform_open01(B[0], B[1]);
+    const double ua = uniform_open01(B[2], B[3]);
+    const double D = __dmul_rn(2.0, p.max_disp);
+    const double tx = __fma_rn(__dadd_rn(ux, -0.5), D, xy.x);
+    const double ty = __fma_rn(__dadd_rn(uy, -0.5), D, xy.y);
+    const double tz = __fma_rn(__dadd_rn(uz, -0.5), D, zq.x);
+    const double a = __dadd_rn(p.R, -p.hh[i]);
+    const double rr = dist2(tx, ty, tz);
+    p.txy[i] = make_double2(tx, ty);
+    p.tz[i] = tz;
+    p.lnu[i] = log(ua);
+    p.wall[i] = (rr > __dmul_rn(a, a)) ? (unsigned char)kFlagWall : (unsigned char)0;
+}
+
+// ------------------------------------------------------------------------------------------
+// a2: bulk pair energy.  Rows = trials of the chunk (one per consumer thread), columns = all
+// particles outside [gap0, gap1) at their current positions, staged through shared memory by
+// 1-D bulk async copies (TMA unit, mbarrier complete_tx) in a kStages ring.  Inner loop is the
+// brush of Alg. 2: every lane reads the same column (smem broadcast).
+// 27 FP64-pipe instructions + 2 MUFU.RSQ64H per pair evaluation.
+// grid = (row groups, slices); block = kBulkRowsPerCta consumers + 1 producer warp.
+// ------------------------------------------------------------------------------------------
+struct __align__(16) ColStage {
+    double2 xy[kColTile];
+    double2 zq[kColTile];
+    double h[kColTile];
+};
+
+__device__ __forceinline__ int slice_bound(int ncols, int nslices, int sl) {
+    return (int)(((long long)(ncols >> 1) * sl) / nslices) << 1;  // even boundaries
+}
+
+__global__ void __launch_bounds__(kBulkRowsPerCta + 32, 2)
+k_bulk(Params p, int row0, int nrows, int gap0, int gap1, int nslices) {
+    __shared__ ColStage stage[kStages];
+    __shared__ __align__(8) uint64_t full_bar[kStages];
+    __shared__ __align__(8) uint64_t empty_bar[kStages];
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    constexpr int kConsumerWarps = kBulkRowsPerCta / 32;
+    const int gap = gap1 - gap0;
+    const int ncols = p.Np - gap;
+    const int sl = blockIdx.y;
+    const int v0 = slice_bound(ncols, nslices, sl), v1 = slice_bound(ncols, nslices, sl + 1);
+
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], kConsumerWarps);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    if (warp == kConsumerWarps) {
+        // ---- producer: one lane walks the slice and feeds the ring ----
+        if (lane == 0) {
+            int k = 0;
+            for (int v = v0; v < v1; ++k) {
+                const int lim = (v < gap0) ? min(v1, gap0) : v1;
+                const int cnt = min(kColTile, lim - v);
+                const int a = (v < gap0) ? v : v + gap;
+                const int s = k % kStages;
+                if (k >= kStages) mbar_wait(&empty_bar[s], ((k / kStages) - 1) & 1);
+                mbar_arrive_expect_tx(&full_bar[s], (uint32_t)cnt * 40u);
+                bulk_g2s(stage[s].xy, p.xy + a, (uint32_t)cnt * 16u, &full_bar[s]);
+                bulk_g2s(stage[s].zq, p.zq + a, (uint32_t)cnt * 16u, &full_bar[s]);
+                bulk_g2s(stage[s].h, p.hh + a, (uint32_t)cnt * 8u, &full_bar[s]);
+                v += cnt;
+            }
+        }
+        return;
+    }
+
+    // ---- consumers: one row per thread ----
+    const int r = blockIdx.x * kBulkRowsPerCta + tid;  // row within the chunk
+    const bool live = r < nrows;
+    const bool warp_live = blockIdx.x * kBulkRowsPerCta + warp * 32 < nrows;  // whole warp past the chunk
+    const int i = row0 + (live ? r : 0);
+    const double2 xyi = p.xy[i];
+    const double2 zqi = p.zq[i];
+    const double2 txyi = p.txy[i];
+    const double xi = xyi.x, yi = xyi.y, zi = zqi.x;
+    const double txi = txyi.x, tyi = txyi.y, tzi = p.tz[i];
+    const double hi = p.hh[i];
+    double acc = 0.0;
+    int ov = 0;
+
+    int k = 0;
+    for (int v = v0; v < v1; ++k) {
+        const int lim = (v < gap0) ? min(v1, gap0) : v1;
+        const int cnt = min(kColTile, lim - v);
+        const int s = k % kStages;
+        mbar_wait(&full_bar[s], (k / kStages) & 1);
+        const ColStage& st = stage[s];
+#pragma unroll 4
+        for (int j = 0; j < (warp_live ? cnt : 0); ++j) {
+            const double2 a = st.xy[j];
+            const double2 b = st.zq[j];
+            const double hj = st.h[j];
+            const double r2o = dist2(__dadd_rn(xi, -a.x), __dadd_rn(yi, -a.y), __dadd_rn(zi, -b.x));
+            const double r2n = dist2(__dadd_rn(txi, -a.x), __dadd_rn(tyi, -a.y), __dadd_rn(tzi, -b.x));
+            const double sij = __dadd_rn(hi, hj);
+            ov += (r2n < __dmul_rn(sij, sij)) ? 1 : 0;
+            const double du = __dadd_rn(rsqrt_fast(r2n), -rsqrt_fast(r2o));
+            acc = __fma_rn(b.y, du, acc);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_bar[s]);
+        v += cnt;
+    }
+    if (live) {
+        p.partA[(size_t)sl * p.chunk + r] = acc;
+        p.ovA[(size_t)sl * p.chunk + r] = ov;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a2/a3 inside the chunk.  One warp per (row tile t, column tile s) of 32 x 32; lane = row.
+//  s > t, or s == t and j > i : partner not yet decided when i is tried -> base term with x_j,
+//                               overlap counted unconditionally.
+//  s < t, or s == t and j < i : partner decided earlier in this chunk.  Base term with the
+//                               chunk-start x_j (as if rejected) and D(i,j) = U(x~_j) - U(x_j)
+//                               to add if j is accepted; overlap bits for both outcomes.
+//    If the trial overlaps x_j the base term is dropped and D = U(x~_j) (i is vetoed anyway
+//    unless j moves away); if it overlaps x~_j, D = 0 (i is vetoed if j is accepted).  So the
+//    energy is exact whenever the trial is not vetoed and no inf/NaN enters a used sum.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int blk_index(int t, int s) { return t * (t + 1) / 2 + s; }
+
+__global__ void __launch_bounds__(256) k_diag(Params p, int row0, int nrows) {
+    __shared__ double2 cxy[8][32], czq[8][32], ctxy[8][32];
+    __shared__ double ch[8][32], ctz[8][32];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nt = nrows / kTile;
+    const int unit = blockIdx.x * 8 + w;
+    if (unit >= nt * nt) return;
+    const int t = unit / nt, s = unit % nt;
+    const int r = t * kTile + lane, i = row0 + r;
+    const int j0 = row0 + s * kTile;
+    cxy[w][lane] = p.xy[j0 + lane];
+    czq[w][lane] = p.zq[j0 + lane];
+    ctxy[w][lane] = p.txy[j0 + lane];
+    ctz[w][lane] = p.tz[j0 + lane];
+    ch[w][lane] = p.hh[j0 + lane];
+    __syncwarp();
+    const double2 xyi = p.xy[i];
+    const double2 txyi = p.txy[i];
+    const double xi = xyi.x, yi = xyi.y, zi = p.zq[i].x;
+    const double txi = txyi.x, tyi = txyi.y, tzi = p.tz[i];
+    const double hi = p.hh[i];
+    const int W = p.chunk / kTile;
+    double bsum = 0.0;
+    int ovc = 0;
+    unsigned ovo = 0u, ovn = 0u;
+    double* blk = (s <= t) ? p.Dblk + (size_t)blk_index(t, s) * (kTile * kTile) : nullptr;
+    for (int jj = 0; jj < kTile; ++jj) {
+        const double2 a = cxy[w][jj];
+        const double2 b = czq[w][jj];
+        const double sij = __dadd_rn(hi, ch[w][jj]);
+        const double s2 = __dmul_rn(sij, sij);
+        const double r2oo = dist2(__dadd_rn(xi, -a.x), __dadd_rn(yi, -a.y), __dadd_rn(zi, -b.x));
+        const double r2no = dist2(__dadd_rn(txi, -a.x), __dadd_rn(tyi, -a.y), __dadd_rn(tzi, -b.x));
+        const bool upper = (s > t) || (s == t && jj > lane);
+        const bool lower = (s < t) || (s == t && jj < lane);
+        if (upper) {
+            bsum = __fma_rn(b.y, __dadd_rn(rsqrt_fast(r2no), -rsqrt_fast(r2oo)), bsum);
+            ovc += (r2no < s2) ? 1 : 0;
+        } else if (lower) {
+            const double2 ta = ctxy[w][jj];
+            const double tzj = ctz[w][jj];
+            const double r2on = dist2(__dadd_rn(xi, -ta.x), __dadd_rn(yi, -ta.y), __dadd_rn(zi, -tzj));
+            const double r2nn = dist2(__dadd_rn(txi, -ta.x), __dadd_rn(tyi, -ta.y), __dadd_rn(tzi, -tzj));
+            const bool oo = r2no < s2, on = r2nn < s2;
+            double uold = 0.0, unew = 0.0;
+            if (!oo) uold = __dmul_rn(b.y, __dadd_rn(rsqrt_fast(r2no), -rsqrt_fast(r2oo)));
+            if (!on) unew = __dmul_rn(b.y, __dadd_rn(rsqrt_fast(r2nn), -rsqrt_fast(r2on)));
+            bsum = __dadd_rn(bsum, uold);
+            const double D = on ? 0.0 : __dadd_rn(unew, -uold);
+            ovo |= (oo ? 1u : 0u) << jj;
+            ovn |= (on ? 1u : 0u) << jj;
+            blk[jj * kTile + lane] = D;
+        } else {
+            blk[jj * kTile + lane] = 0.0;  // jj == lane on the diagonal block
+        }
+        if (s == t && jj > lane) blk[jj * kTile + lane] = 0.0;
+    }
+    p.partD[(size_t)s * p.chunk + r] = bsum;
+    p.ovD[(size_t)s * p.chunk + r] = ovc;
+    if (s <= t) {
+        p.OVold[(size_t)r * W + s] = ovo;
+        p.OVnew[(size_t)r * W + s] = ovn;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a3/a4: sequential resolution of one chunk (Alg. 4).
+// One CTA.  Warp 0 is the chain: lane l owns particle 32t+l of tile t; step j = lane j's
+// decision, published by __ballot_sync; lanes > j add their precomputed D(l,j) if j accepted.
+// Then all warps propagate the tile's accept mask to the rows of later tiles (block column
+// t of D), and the last warp prefetches the next diagonal block.
+// accept iff no veto and l_B q_i sum + ln u < 0 (Eq. 1 in log form, strict; G3, G4).
+// ------------------------------------------------------------------------------------------
+constexpr int kChainThreads = 512;
+
+__global__ void __launch_bounds__(kChainThreads, 1)
+k_chain(Params p, int row0, int nrows, int nslices, int last_chunk) {
+    __shared__ double sE[kChunkMax];
+    __shared__ unsigned char sVeto[kChunkMax];
+    __shared__ double sDiag[2][kTile * kTile];      // diagonal D block of tile t (double buffered)
+    __shared__ double sLbq[2][kTile], sLnu[2][kTile];
+    __shared__ unsigned sOvo[2][kTile], sOvn[2][kTile];
+    __shared__ unsigned sA;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    constexpr int nwarps = kChainThreads / 32;
+    const int nt = nrows / kTile;
+    const int W = p.chunk / kTile;
+
+    // prologue: reduce the partial sums in a fixed order
+    for (int r = tid; r < nrows; r += kChainThreads) {
+        double e = 0.0;
+        int ov = 0;
+        for (int sl = 0; sl < nslices; ++sl) {
+            e += p.partA[(size_t)sl * p.chunk + r];
+            ov += p.ovA[(size_t)sl * p.chunk + r];
+        }
+        for (int s = 0; s < nt; ++s) {
+            e += p.partD[(size_t)s * p.chunk + r];
+            ov += p.ovD[(size_t)s * p.chunk + r];
+        }
+        const int i = row0 + r;
+        sE[r] = e;
+        sVeto[r] = (unsigned char)(p.wall[i] | (ov > 0 ? kFlagOverlap : 0u));
+    }
+    for (int e = tid; e < kTile * kTile; e += kChainThreads) sDiag[0][e] = p.Dblk[e];
+    if (tid < kTile) {
+        sLbq[0][tid] = p.lbq[row0 + tid];
+        sLnu[0][tid] = p.lnu[row0 + tid];
+        sOvo[0][tid] = p.OVold[(size_t)tid * W];
+        sOvn[0][tid] = p.OVnew[(size_t)tid * W];
+    }
+    __syncthreads();
+
+    unsigned long long n_acc = 0, n_ov = 0, n_wall = 0, n_tie = 0;
+    double e_run = 0.0;
+
+    for (int t = 0; t < nt; ++t) {
+        if (warp == 0) {
+            const int r = t * kTile + lane, i = row0 + r;
+            const double* dg = sDiag[t & 1];
+            const double lbq = sLbq[t & 1][lane], lnu = sLnu[t & 1][lane];
+            double Eu = sE[r];
+            double Es = __fma_rn(lbq, Eu, lnu);
+            const unsigned vflags = sVeto[r];
+            const bool wallv = (vflags & kFlagWall) != 0u;
+            bool ovv = (vflags & kFlagOverlap) != 0u;
+            const unsigned ovo = sOvo[t & 1][lane], ovn = sOvn[t & 1][lane];
+            unsigned A = 0u;
+#pragma unroll
+            for (int j = 0; j < kTile; ++j) {
+                const double dj = dg[j * kTile + lane];       // 0 for lanes <= j
+                const double djs = __dmul_rn(lbq, dj);
+                const bool ok = !wallv && !ovv && (Es < 0.0);
+                const unsigned bal = __ballot_sync(0xffffffffu, ok);
+                const bool bit = ((bal >> j) & 1u) != 0u;
+                A |= (bit ? 1u : 0u) << j;
+                if (bit) {
+                    Es = __dadd_rn(Es, djs);
+                    Eu = __dadd_rn(Eu, dj);
+                }
+                ovv = ovv || ((((bit ? ovn : ovo) >> j) & 1u) != 0u);  // bits >= lane are 0
+            }
+            const bool acc = ((A >> lane) & 1u) != 0u;
+            const double dE = __dmul_rn(lbq, Eu);
+            const bool tie = !wallv && !ovv && (fabs(Es) < 1e-8);
+            if (acc) {
+                const double2 txy = p.txy[i];
+                const double tz = p.tz[i];
+                const double q = p.zq[i].y;
+                p.xy[i] = txy;
+                p.zq[i] = make_double2(tz, q);
+            }
+            p.log_dE[i] = dE;
+            p.log_flags[i] = (unsigned char)((acc ? kFlagAccept : 0u) | (ovv ? kFlagOverlap : 0u) |
+                                             (wallv ? kFlagWall : 0u) | (tie ? kFlagNearTie : 0u));
+            const bool real = i < p.N;
+            n_acc += __popc(A);
+            n_ov += __popc(__ballot_sync(0xffffffffu, real && ovv));
+            n_wall += __popc(__ballot_sync(0xffffffffu, real && wallv));
+            n_tie += __popc(__ballot_sync(0xffffffffu, real && tie));
+            e_run += warp_sum(acc ? dE : 0.0);
+            if (lane == 0) sA = A;
+        }
+        __syncthreads();
+        const unsigned A = sA;
+        // propagate to later tiles: rows of tile t2 get sum over accepted jj of D(t2, t)[jj][lane]
+        for (int t2 = t + 1 + warp; t2 < nt; t2 += nwarps) {
+            const int r = t2 * kTile + lane;
+            const double* blk = p.Dblk + (size_t)blk_index(t2, t) * (kTile * kTile);
+            double e = sE[r];
+#pragma unroll 8
+            for (int jj = 0; jj < kTile; ++jj)
+                if ((A >> jj) & 1u) e = __dadd_rn(e, blk[jj * kTile + lane]);
+            sE[r] = e;
+            const unsigned on = p.OVnew[(size_t)r * W + t], oo = p.OVold[(size_t)r * W + t];
+            if (((on & A) | (oo & ~A)) != 0u) sVeto[r] |= (unsigned char)kFlagOverlap;
+        }
+        if (warp == nwarps - 1 && t + 1 < nt) {
+            const double* nb = p.Dblk + (size_t)blk_index(t + 1, t + 1) * (kTile * kTile);
+            double* dst = sDiag[(t + 1) & 1];
+            for (int e = lane; e < kTile * kTile; e += 32) dst[e] = nb[e];
+            const int rn = (t + 1) * kTile + lane;
+            sLbq[(t + 1) & 1][lane] = p.lbq[row0 + rn];
+            sLnu[(t + 1) & 1][lane] = p.lnu[row0 + rn];
+            sOvo[(t + 1) & 1][lane] = p.OVold[(size_t)rn * W + t + 1];
+            sOvn[(t + 1) & 1][lane] = p.OVnew[(size_t)rn * W + t + 1];
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        DevState* st = p.st;
+        st->accepted += n_acc;
+        st->veto_overlap += n_ov;
+        st->veto_wall += n_wall;
+        st->near_ties += n_tie;
+        st->E_run += e_run;
+        if (last_chunk) st->sweep += 1ull;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// packing between the caller's SoA [3][N] and the workspace layout
+// ------------------------------------------------------------------------------------------
+__global__ void k_pack(Params p, const double* pos, const double* q, const double* d) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.Np) return;
+    if (i < p.N) {
+        p.xy[i] = make_double2(pos[i], pos[(size_t)p.N + i]);
+        if (q) {
+            p.zq[i] = make_double2(pos[2 * (size_t)p.N + i], q[i]);
+            p.hh[i] = __dmul_rn(0.5, d[i]);
+            p.lbq[i] = __dmul_rn(p.lB, q[i]);
+        } else {
+            p.zq[i].x = pos[2 * (size_t)p.N + i];
+        }
+    } else if (q) {
+        p.xy[i] = make_double2(kGhostCoord + kGhostStep * (double)(i - p.N), 0.0);
+        p.zq[i] = make_double2(0.0, 0.0);
+        p.hh[i] = 0.0;
+        p.lbq[i] = 0.0;
+    }
+}
+
+__global__ void k_unpack(Params p, double* pos) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.N) return;
+    const double2 xy = p.xy[i];
+    pos[i] = xy.x;
+    pos[(size_t)p.N + i] = xy.y;
+    pos[2 * (size_t)p.N + i] = p.zq[i].x;
+}
+
+__global__ void k_set_sweep(DevState* st, unsigned long long s) { st->sweep = s; }
+
+__global__ void k_copy_log(Params p, double* dE, unsigned char* flags) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.N) return;
+    if (dE) dE[i] = p.log_dE[i];
+    if (flags) flags[i] = p.log_flags[i];
+}
+
+// per-particle input checks: finite, d > 0, inside the wall
+__global__ void k_check_particles(Params p, const double* d) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.N) return;
+    const double2 xy = p.xy[i];
+    const double2 zq = p.zq[i];
+    const double di = d[i];
+    int err = 0;
+    if (!isfinite(xy.x) || !isfinite(xy.y) || !isfinite(zq.x) || !isfinite(zq.y) || !isfinite(di) ||
+        !(di > 0.0)) {
+        err = -1;
+    } else {
+        const double a = __dadd_rn(p.R, -p.hh[i]);
+        if (!(a >= 0.0) || dist2(xy.x, xy.y, zq.x) > __dmul_rn(a, a)) err = -3;
+    }
+    if (err) atomicMin(&p.st->err, err == -1 ? -1000 : err);  // EINVAL outranks the others
+}
+
+// ------------------------------------------------------------------------------------------
+// a5: from-scratch energy (and the overlap check of mc_init).  Row i sums q_j / r_ij over
+// j > i; columns are cut in 256-wide tiles handed round-robin to gridDim.y slices.
+// part[slice][i] is reduced in fixed order by k_energy_reduce.
+// ------------------------------------------------------------------------------------------
+constexpr int kEnergySlices = 32;
+
+__global__ void __launch_bounds__(256) k_energy(Params p, double* part, int check_overlap) {
+    __shared__ double2 sxy[256], szq[256];
+    __shared__ double sh[256];
+    const int tid = threadIdx.x;
+    const int rg = blockIdx.x, sl = blockIdx.y;
+    const int i = rg * 256 + tid;
+    const bool live = i < p.Np;
+    double2 xyi = make_double2(0, 0), zqi = make_double2(0, 0);
+    double hi = 0;
+    if (live) { xyi = p.xy[i]; zqi = p.zq[i]; hi = p.hh[i]; }
+    double acc = 0.0;
+    int bad = 0;
+    const int ntile = (p.Np + 255) / 256;
+    for (int ct = rg + sl; ct < ntile; ct += kEnergySlices) {
+        const int j0 = ct * 256;
+        __syncthreads();
+        if (j0 + tid < p.Np) { sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; sh[tid] = p.hh[j0 + tid]; }
+        __syncthreads();
+        const int cnt = min(256, p.Np - j0);
+        if (!live) continue;
+#pragma unroll 4
+        for (int j = 0; j < cnt; ++j) {
+            if (j0 + j <= i) continue;
+            const double2 a = sxy[j], b = szq[j];
+            const double r2 = dist2(__dadd_rn(xyi.x, -a.x), __dadd_rn(xyi.y, -a.y), __dadd_rn(zqi.x, -b.x));
+            acc = __fma_rn(b.y, rsqrt_fast(r2), acc);
+            if (check_overlap) {
+                const double sij = __dadd_rn(hi, sh[j]);
+                bad |= (r2 < __dmul_rn(sij, sij)) && (j0 + j < p.N) && (i < p.N);
+            }
+        }
+    }
+    if (live) part[(size_t)sl * p.Np + i] = __dmul_rn(zqi.y, acc);
+    if (bad) atomicMin(&p.st->err, -2);
+}
+
+// out = l_B * sum_i sum_slices part; optionally stored into E_run.  One CTA of 1024 threads.
+__global__ void __launch_bounds__(1024) k_energy_reduce(Params p, const double* part, double* out,
+                                                        int set_running) {
+    __shared__ double red[1024];
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < p.Np; i += 1024)
+        for (int sl = 0; sl < kEnergySlices; ++sl) acc += part[(size_t)sl * p.Np + i];
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const double E = __dmul_rn(p.lB, red[0]);
+        if (out) *out = E;
+        if (set_running) p.st->E_run = E;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a6: pair-distance histograms.  k_centres lists the bulk ions in
+// index order; k_hist bins (centre, any partner) distances into shared-memory histograms.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) k_centres(Params p, double centre_rmax, int* list, int* count,
+                                                  unsigned long long* n_centres) {
+    __shared__ int wcount[32];
+    __shared__ int base;
+    __shared__ unsigned long long nsp[2];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) { base = 0; nsp[0] = nsp[1] = 0ull; }
+    __syncthreads();
+    const double c2 = __dmul_rn(centre_rmax, centre_rmax);
+    for (int i0 = 0; i0 < p.N; i0 += 1024) {
+        const int i = i0 + tid;
+        bool is = false;
+        int sp = 0;
+        if (i < p.N) {
+            const double2 xy = p.xy[i];
+            const double2 zq = p.zq[i];
+            is = dist2(xy.x, xy.y, zq.x) <= c2;
+            sp = zq.y > 0.0 ? 0 : 1;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, is);
+        const unsigned m0 = __ballot_sync(0xffffffffu, is && sp == 0);
+        if (lane == 0) wcount[warp] = __popc(m);
+        __syncthreads();
+        int off = base;
+        for (int w = 0; w < warp; ++w) off += wcount[w];
+        if (is) list[off + __popc(m & ((1u << lane) - 1u))] = i;
+        if (lane == 0) {
+            atomicAdd(&nsp[0], (unsigned long long)__popc(m0));
+            atomicAdd(&nsp[1], (unsigned long long)(__popc(m) - __popc(m0)));
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int tot = 0;
+            for (int w = 0; w < 32; ++w) tot += wcount[w];
+            base += tot;
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        *count = base;
+        n_centres[0] += nsp[0];
+        n_centres[1] += nsp[1];
+    }
+}
+
+constexpr int kHistSlices = 16;
+
+__global__ void __launch_bounds__(256) k_hist(Params p, const int* list, const int* count, double inv_w,
+                                              int nbins, double cut2, unsigned long long* hist) {
+    extern __shared__ unsigned shist[];  // [4][nbins]
+    __shared__ double2 sxy[256], szq[256];
+    const int tid = threadIdx.x;
+    const int nc = *count;
+    if ((int)blockIdx.x * 256 >= nc) return;
+    for (int b = tid; b < 4 * nbins; b += 256) shist[b] = 0u;
+    const int c = blockIdx.x * 256 + tid;
+    const bool live = c < nc;
+    const int i = live ? list[c] : -1;
+    double2 xyi = make_double2(0, 0), zqi = make_double2(0, 0);
+    if (live) { xyi = p.xy[i]; zqi = p.zq[i]; }
+    const int si = zqi.y > 0.0 ? 0 : 1;
+    const int ntile = (p.N + 255) / 256;
+    for (int ct = blockIdx.y; ct < ntile; ct += kHistSlices) {
+        const int j0 = ct * 256;
+        __syncthreads();
+        if (j0 + tid < p.N) { sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; }
+        __syncthreads();
+        const int cnt = min(256, p.N - j0);
+        if (!live) continue;
+#pragma unroll 4
+        for (int j = 0; j < cnt; ++j) {
+            const double2 a = sxy[j], b = szq[j];
+            const double r2 = dist2(__dadd_rn(xyi.x, -a.x), __dadd_rn(xyi.y, -a.y), __dadd_rn(zqi.x, -b.x));
+            if (r2 < cut2 && (j0 + j) != i) {
+                const double fb = floor(__dmul_rn(sqrt(r2), inv_w));
+                if (fb < (double)nbins) {
+                    const int sj = b.y > 0.0 ? 0 : 1;
+                    atomicAdd(&shist[(si * 2 + sj) * nbins + (int)fb], 1u);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int b = tid; b < 4 * nbins; b += 256) {
+        const unsigned v = shist[b];
+        if (v) atomicAdd(&hist[b], (unsigned long long)v);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// FP64 peak probe: 8 independent DFMA chains per thread, register resident.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_dfma_peak(double* sink, int iters) {
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
+           a7 = a0 + 7;
+    const double m = 1.0000001, c = 1e-9;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            a0 = __fma_rn(a0, m, c); a1 = __fma_rn(a1, m, c); a2 = __fma_rn(a2, m, c); a3 = __fma_rn(a3, m, c);
+            a4 = __fma_rn(a4, m, c); a5 = __fma_rn(a5, m, c); a6 = __fma_rn(a6, m, c); a7 = __fma_rn(a7, m, c);
+        }
+    }
+    const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 123.456) sink[0] = s;
+}
+
+}  // namespace mcb

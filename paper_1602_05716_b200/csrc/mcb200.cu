@@ -1,0 +1,430 @@
+// mcb200.cu -- host side of libmcb200.so: the C ABI declared in include/mcb200.h.
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -fmad=false -shared -Xcompiler -fPIC
+#include "../../include/mcb200.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace mcb;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                           \
+    do {                                                                                         \
+        cudaError_t e_ = (expr);                                                                 \
+        if (e_ != cudaSuccess)                                                                   \
+            return fail(MC_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));           \
+    } while (0)
+
+constexpr size_t kAlign = 256;
+size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {
+    size_t xy, zq, hh, lbq, txy, tz, lnu, wall, partA, ovA, partD, ovD, Dblk, OVold, OVnew, log_dE, log_flags,
+        st, epart, centres, ccount, stage_pos, total;
+};
+
+int padded(int64_t N) { return (int)((N + kTile - 1) / kTile * kTile); }
+
+Layout make_layout(int64_t N) {
+    Layout L{};
+    const size_t Np = (size_t)padded(N);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    const size_t nt = kChunkMax / kTile;
+    L.xy = take(Np * 16); L.zq = take(Np * 16); L.hh = take(Np * 8); L.lbq = take(Np * 8);
+    L.txy = take(Np * 16); L.tz = take(Np * 8); L.lnu = take(Np * 8); L.wall = take(Np);
+    L.partA = take((size_t)kMaxSlices * kChunkMax * 8); L.ovA = take((size_t)kMaxSlices * kChunkMax * 4);
+    L.partD = take(nt * kChunkMax * 8); L.ovD = take(nt * kChunkMax * 4);
+    L.Dblk = take(nt * (nt + 1) / 2 * kTile * kTile * 8);
+    L.OVold = take((size_t)kChunkMax * nt * 4); L.OVnew = take((size_t)kChunkMax * nt * 4);
+    L.log_dE = take(Np * 8); L.log_flags = take(Np);
+    L.st = take(sizeof(DevState));
+    L.epart = take((size_t)kEnergySlices * Np * 8 + 8);
+    L.centres = take(Np * 4); L.ccount = take(16);
+    L.stage_pos = take(3 * (size_t)N * 8);
+    L.total = off;
+    return L;
+}
+
+}  // namespace
+
+struct mc_handle {
+    Params p{};
+    Layout L{};
+    char* ws = nullptr;
+    cudaStream_t stream = nullptr;
+    cudaStream_t cap_stream = nullptr;
+    int num_sms = 148;
+    int chunk = kChunkMax;
+    bool use_graph = true;
+    bool overlap = false;
+    cudaGraphExec_t graph = nullptr;
+    uint64_t launches = 0;
+    uint64_t launches_per_sweep = 0;
+    double* epart = nullptr;
+    int* centres = nullptr;
+    int* ccount = nullptr;
+    double* stage_pos = nullptr;
+};
+
+namespace {
+
+void drop_graph(mc_handle* h) {
+    if (h->graph) {
+        cudaGraphExecDestroy(h->graph);
+        h->graph = nullptr;
+    }
+}
+
+int slices_for(const mc_handle* h, int nrows, int ncols) {
+    const int rgs = (nrows + kBulkRowsPerCta - 1) / kBulkRowsPerCta;
+    int target = (2 * h->num_sms + rgs - 1) / rgs;      // two CTAs per SM
+    const int max_by_cols = ncols / 64 > 0 ? ncols / 64 : 1;  // at least 64 columns per slice
+    if (target > max_by_cols) target = max_by_cols;
+    if (target > kMaxSlices) target = kMaxSlices;
+    if (target < 1) target = 1;
+    return target;
+}
+
+// Enqueue one sweep on `s`.  Returns the number of kernels launched.
+int enqueue_sweep(mc_handle* h, cudaStream_t s, uint64_t* count) {
+    Params p = h->p;
+    p.chunk = h->chunk;
+    uint64_t n = 0;
+    k_trial<<<(p.Np + 255) / 256, 256, 0, s>>>(p);
+    ++n;
+    const int nchunks = (p.Np + h->chunk - 1) / h->chunk;
+    for (int c = 0; c < nchunks; ++c) {
+        const int row0 = c * h->chunk;
+        const int nrows = std::min(h->chunk, p.Np - row0);
+        const int ncols = p.Np - nrows;
+        int nslices = 0;
+        if (ncols > 0) {
+            nslices = slices_for(h, nrows, ncols);
+            dim3 grid((nrows + kBulkRowsPerCta - 1) / kBulkRowsPerCta, nslices);
+            k_bulk<<<grid, kBulkRowsPerCta + 32, 0, s>>>(p, row0, nrows, row0, row0 + nrows, nslices);
+            ++n;
+        }
+        const int nt = nrows / kTile;
+        k_diag<<<(nt * nt + 7) / 8, 256, 0, s>>>(p, row0, nrows);
+        ++n;
+        k_chain<<<1, kChainThreads, 0, s>>>(p, row0, nrows, nslices, c == nchunks - 1 ? 1 : 0);
+        ++n;
+    }
+    if (count) *count = n;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(MC_ECUDA, std::string("sweep launch: ") + cudaGetErrorString(e));
+    return MC_OK;
+}
+
+int build_graph(mc_handle* h) {
+    drop_graph(h);
+    cudaGraph_t g = nullptr;
+    // capture on a private stream (the caller's may be the legacy default stream, which cannot capture)
+    if (!h->cap_stream) CUDA_TRY(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    CUDA_TRY(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+    uint64_t n = 0;
+    const int rc = enqueue_sweep(h, h->cap_stream, &n);
+    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
+    if (rc != MC_OK) {
+        if (g) cudaGraphDestroy(g);
+        return rc;
+    }
+    if (e != cudaSuccess) return fail(MC_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+    e = cudaGraphInstantiate(&h->graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) return fail(MC_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e));
+    h->launches_per_sweep = n;
+    return MC_OK;
+}
+
+int enqueue_energy(mc_handle* h, double* out_dev, int set_running, int check_overlap) {
+    const Params& p = h->p;
+    dim3 grid((p.Np + 255) / 256, kEnergySlices);
+    k_energy<<<grid, 256, 0, h->stream>>>(p, h->epart, check_overlap);
+    k_energy_reduce<<<1, 1024, 0, h->stream>>>(p, h->epart, out_dev, set_running);
+    h->launches += 2;
+    CUDA_TRY(cudaGetLastError());
+    return MC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mc_last_error(void) { return g_err.c_str(); }
+
+size_t mc_workspace_bytes(int64_t N) {
+    if (N < 1 || N > (int64_t)1 << 30) return 0;
+    return make_layout(N).total;
+}
+
+int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* charges_dev,
+            const double* diameters_dev, double cavity_R, double bjerrum_length, double max_disp, uint64_t seed,
+            void* workspace_dev, size_t workspace_bytes, void* stream, int validate) {
+    if (!out) return fail(MC_EINVAL, "out is null");
+    *out = nullptr;
+    if (N < 1 || N > (int64_t)1 << 30) return fail(MC_EINVAL, "N out of range");
+    if (!pos_dev || !charges_dev || !diameters_dev || !workspace_dev) return fail(MC_EINVAL, "null pointer");
+    if (!(cavity_R > 0) || !(bjerrum_length >= 0) || !(max_disp >= 0) || !std::isfinite(cavity_R) ||
+        !std::isfinite(bjerrum_length) || !std::isfinite(max_disp))
+        return fail(MC_EINVAL, "cavity_R must be > 0, bjerrum_length >= 0, max_disp >= 0, all finite");
+    if (((uintptr_t)workspace_dev % kAlign) != 0) return fail(MC_EINVAL, "workspace must be 256-byte aligned");
+    const Layout L = make_layout(N);
+    if (workspace_bytes < L.total) return fail(MC_ENOSPACE, "workspace smaller than mc_workspace_bytes(N)");
+
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    cudaDeviceProp prop{};
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) return fail(MC_ECUDA, "libmcb200 needs an sm_100 device (B200); found sm_" +
+                                                    std::to_string(prop.major) + std::to_string(prop.minor));
+
+    mc_handle* h = new mc_handle;
+    h->L = L;
+    h->ws = (char*)workspace_dev;
+    h->stream = (cudaStream_t)stream;
+    h->num_sms = prop.multiProcessorCount;
+    Params& p = h->p;
+    p.N = (int)N; p.Np = padded(N); p.chunk = h->chunk;
+    char* w = h->ws;
+    p.xy = (double2*)(w + L.xy); p.zq = (double2*)(w + L.zq); p.hh = (double*)(w + L.hh);
+    p.lbq = (double*)(w + L.lbq); p.txy = (double2*)(w + L.txy); p.tz = (double*)(w + L.tz);
+    p.lnu = (double*)(w + L.lnu); p.wall = (unsigned char*)(w + L.wall);
+    p.partA = (double*)(w + L.partA); p.ovA = (int*)(w + L.ovA);
+    p.partD = (double*)(w + L.partD); p.ovD = (int*)(w + L.ovD);
+    p.Dblk = (double*)(w + L.Dblk); p.OVold = (unsigned*)(w + L.OVold); p.OVnew = (unsigned*)(w + L.OVnew);
+    p.log_dE = (double*)(w + L.log_dE); p.log_flags = (unsigned char*)(w + L.log_flags);
+    p.st = (DevState*)(w + L.st);
+    p.R = cavity_R; p.lB = bjerrum_length; p.max_disp = max_disp; p.seed = seed;
+    h->epart = (double*)(w + L.epart);
+    h->centres = (int*)(w + L.centres);
+    h->ccount = (int*)(w + L.ccount);
+    h->stage_pos = (double*)(w + L.stage_pos);
+
+    auto bail = [&](int code) { delete h; return code; };
+    cudaError_t e = cudaMemsetAsync(w, 0, L.total, h->stream);
+    if (e != cudaSuccess) return bail(fail(MC_ECUDA, std::string("memset: ") + cudaGetErrorString(e)));
+    const int nb = (p.Np + 255) / 256;
+    k_pack<<<nb, 256, 0, h->stream>>>(p, pos_dev, charges_dev, diameters_dev);
+    k_check_particles<<<nb, 256, 0, h->stream>>>(p, diameters_dev);
+    h->launches += 2;
+    if (validate) {
+        const int rc = enqueue_energy(h, nullptr, 1, 1);
+        if (rc != MC_OK) return bail(rc);
+    }
+    DevState st{};
+    e = cudaMemcpyAsync(&st, p.st, sizeof(st), cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return bail(fail(MC_ECUDA, std::string("init: ") + cudaGetErrorString(e)));
+    if (st.err != 0) {
+        if (st.err <= -1000) return bail(fail(MC_EINVAL, "non-finite input or diameter <= 0"));
+        if (st.err == -3) return bail(fail(MC_EOUTSIDE, "an ion sticks out of the cavity"));
+        return bail(fail(MC_EOVERLAP, "two ions overlap in the initial configuration"));
+    }
+    *out = h;
+    return MC_OK;
+}
+
+int mc_free(mc_handle* h) {
+    if (!h) return MC_OK;
+    cudaStreamSynchronize(h->stream);
+    drop_graph(h);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    delete h;
+    return MC_OK;
+}
+
+int mc_sweep(mc_handle* h, int64_t n) {
+    if (!h || n < 0) return fail(MC_EINVAL, "bad handle or n < 0");
+    if (n == 0) return MC_OK;
+    if (h->use_graph) {
+        if (!h->graph) {
+            const int rc = build_graph(h);
+            if (rc != MC_OK) return rc;
+        }
+        for (int64_t s = 0; s < n; ++s) CUDA_TRY(cudaGraphLaunch(h->graph, h->stream));
+        h->launches += h->launches_per_sweep * (uint64_t)n;
+    } else {
+        for (int64_t s = 0; s < n; ++s) {
+            uint64_t c = 0;
+            const int rc = enqueue_sweep(h, h->stream, &c);
+            if (rc != MC_OK) return rc;
+            h->launches += c;
+        }
+    }
+    return MC_OK;
+}
+
+int mc_energy(mc_handle* h, double* E_host) {
+    if (!h || !E_host) return fail(MC_EINVAL, "null argument");
+    double* out = h->epart + (size_t)kEnergySlices * h->p.Np;
+    const int rc = enqueue_energy(h, out, 0, 0);
+    if (rc != MC_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(E_host, out, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return MC_OK;
+}
+
+int mc_pair_hist(mc_handle* h, double bin_width, int nbins, double centre_rmax, uint64_t* hist_dev,
+                 uint64_t* n_centres_dev) {
+    if (!h || !hist_dev || !n_centres_dev) return fail(MC_EINVAL, "null argument");
+    if (!(bin_width > 0) || nbins < 1 || nbins > 8192 || !(centre_rmax >= 0))
+        return fail(MC_EINVAL, "bin_width > 0, 1 <= nbins <= 8192, centre_rmax >= 0 required");
+    const Params& p = h->p;
+    const double inv_w = 1.0 / bin_width;
+    const double rcut = (double)nbins * bin_width * (1.0 + 1e-9);
+    const double cut2 = rcut * rcut;
+    k_centres<<<1, 1024, 0, h->stream>>>(p, centre_rmax, h->centres, h->ccount,
+                                         (unsigned long long*)n_centres_dev);
+    const size_t smem = (size_t)4 * nbins * sizeof(unsigned);
+    if (smem > 40 * 1024)
+        CUDA_TRY(cudaFuncSetAttribute(k_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dim3 grid((p.N + 255) / 256, kHistSlices);
+    k_hist<<<grid, 256, smem, h->stream>>>(p, h->centres, h->ccount, inv_w, nbins, cut2,
+                                           (unsigned long long*)hist_dev);
+    h->launches += 2;
+    CUDA_TRY(cudaGetLastError());
+    return MC_OK;
+}
+
+int mc_get_positions(mc_handle* h, double* pos_dev_out) {
+    if (!h || !pos_dev_out) return fail(MC_EINVAL, "null argument");
+    k_unpack<<<(h->p.N + 255) / 256, 256, 0, h->stream>>>(h->p, pos_dev_out);
+    h->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    return MC_OK;
+}
+
+int mc_set_positions(mc_handle* h, const double* pos_dev) {
+    if (!h || !pos_dev) return fail(MC_EINVAL, "null argument");
+    k_pack<<<(h->p.Np + 255) / 256, 256, 0, h->stream>>>(h->p, pos_dev, nullptr, nullptr);
+    h->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    return enqueue_energy(h, nullptr, 1, 0);
+}
+
+int mc_get_sweep_index(mc_handle* h, uint64_t* s_host) {
+    if (!h || !s_host) return fail(MC_EINVAL, "null argument");
+    unsigned long long s = 0;
+    CUDA_TRY(cudaMemcpyAsync(&s, &h->p.st->sweep, sizeof(s), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    *s_host = s;
+    return MC_OK;
+}
+
+int mc_set_sweep_index(mc_handle* h, uint64_t s) {
+    if (!h) return fail(MC_EINVAL, "null handle");
+    k_set_sweep<<<1, 1, 0, h->stream>>>(h->p.st, (unsigned long long)s);
+    h->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    return MC_OK;
+}
+
+int mc_get_stats(mc_handle* h, mc_stats* stats_host) {
+    if (!h || !stats_host) return fail(MC_EINVAL, "null argument");
+    DevState st{};
+    CUDA_TRY(cudaMemcpyAsync(&st, h->p.st, sizeof(st), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    stats_host->accepted = st.accepted; stats_host->veto_overlap = st.veto_overlap;
+    stats_host->veto_wall = st.veto_wall; stats_host->near_ties = st.near_ties;
+    stats_host->E_running = st.E_run;
+    return MC_OK;
+}
+
+int mc_get_trial_log(mc_handle* h, double* dE_dev, uint8_t* flags_dev) {
+    if (!h) return fail(MC_EINVAL, "null handle");
+    k_copy_log<<<(h->p.N + 255) / 256, 256, 0, h->stream>>>(h->p, dE_dev, flags_dev);
+    h->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    return MC_OK;
+}
+
+int mc_sweep_host(mc_handle* h, int64_t n, const double* pos_in_host, double* pos_out_host,
+                  mc_stats* stats_host) {
+    if (!h || n < 0) return fail(MC_EINVAL, "bad handle or n < 0");
+    const size_t bytes = 3 * (size_t)h->p.N * sizeof(double);
+    if (pos_in_host) {
+        CUDA_TRY(cudaMemcpyAsync(h->stage_pos, pos_in_host, bytes, cudaMemcpyHostToDevice, h->stream));
+        const int rc = mc_set_positions(h, h->stage_pos);
+        if (rc != MC_OK) return rc;
+    }
+    int rc = mc_sweep(h, n);
+    if (rc != MC_OK) return rc;
+    if (pos_out_host) {
+        rc = mc_get_positions(h, h->stage_pos);
+        if (rc != MC_OK) return rc;
+        CUDA_TRY(cudaMemcpyAsync(pos_out_host, h->stage_pos, bytes, cudaMemcpyDeviceToHost, h->stream));
+    }
+    if (stats_host) return mc_get_stats(h, stats_host);
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return MC_OK;
+}
+
+int mc_measure_fp64_peak(void* stream, double millis, double* dfma_per_second_host) {
+    if (!dfma_per_second_host || !(millis > 0)) return fail(MC_EINVAL, "bad argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    cudaDeviceProp prop{};
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    const int blocks = prop.multiProcessorCount * 8;
+    cudaEvent_t a, b;
+    CUDA_TRY(cudaEventCreate(&a));
+    CUDA_TRY(cudaEventCreate(&b));
+    int iters = 2000;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        CUDA_TRY(cudaEventRecord(a, s));
+        k_dfma_peak<<<blocks, 256, 0, s>>>(nullptr, iters);
+        CUDA_TRY(cudaEventRecord(b, s));
+        CUDA_TRY(cudaEventSynchronize(b));
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, a, b));
+        const double ops = (double)blocks * 256.0 * (double)iters * 64.0;
+        if (rep > 0 && ms > 0.f) best = std::max(best, ops / (ms * 1e-3));
+        if (ms > 0.f && rep == 0) iters = (int)std::min(4.0e6, std::max(2000.0, iters * millis / ms));
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    CUDA_TRY(cudaGetLastError());
+    *dfma_per_second_host = best;
+    return MC_OK;
+}
+
+int mc_set_option(mc_handle* h, const char* key, int64_t value) {
+    if (!h || !key) return fail(MC_EINVAL, "null argument");
+    if (!std::strcmp(key, "chunk")) {
+        if (value < kTile || value > kChunkMax || value % kTile) return fail(MC_EINVAL, "chunk must be a multiple of 32 in 32..1024");
+        h->chunk = (int)value;
+    } else if (!std::strcmp(key, "graph")) {
+        h->use_graph = value != 0;
+    } else if (!std::strcmp(key, "overlap")) {
+        h->overlap = value != 0;
+    } else {
+        return fail(MC_EINVAL, std::string("unknown option ") + key);
+    }
+    drop_graph(h);
+    return MC_OK;
+}
+
+int mc_get_launch_count(mc_handle* h, uint64_t* n_host) {
+    if (!h || !n_host) return fail(MC_EINVAL, "null argument");
+    *n_host = h->launches;
+    return MC_OK;
+}
+
+}  // extern "C"
