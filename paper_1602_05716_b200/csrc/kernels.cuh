@@ -75,6 +75,7 @@ __global__ void __launch_bounds__(256) k_trial(Params p) {
 // brush of Alg. 2: every lane reads the same column (smem broadcast).
 // 27 FP64-pipe instructions + 2 MUFU.RSQ64H per pair evaluation.
 // grid = (row groups, slices); block = kBulkRowsPerCta consumers + 1 producer warp.
+// Partial sums go to slots slot0 .. slot0+nslices-1 of partA / ovA.
 // ------------------------------------------------------------------------------------------
 struct __align__(16) ColStage {
     double2 xy[kColTile];
@@ -87,15 +88,18 @@ __device__ __forceinline__ int slice_bound(int ncols, int nslices, int sl) {
 }
 
 __global__ void __launch_bounds__(kBulkRowsPerCta + 32, 2)
-k_bulk(Params p, int row0, int nrows, int gap0, int gap1, int nslices) {
+k_bulk(Params p, int row0, int nrows, int cbeg, int cend, int gap0, int gap1, int nslices, int slot0) {
     __shared__ ColStage stage[kStages];
     __shared__ __align__(8) uint64_t full_bar[kStages];
     __shared__ __align__(8) uint64_t empty_bar[kStages];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int kConsumerWarps = kBulkRowsPerCta / 32;
+    // columns = [cbeg, cend) minus [gap0, gap1) (gap inside the range, or empty), as a virtual
+    // index space v in [0, ncols): actual column = cbeg + v (+ gap if at or past the gap)
     const int gap = gap1 - gap0;
-    const int ncols = p.Np - gap;
+    const int ncols = (cend - cbeg) - gap;
+    const int gapv = gap0 - cbeg;
     const int sl = blockIdx.y;
     const int v0 = slice_bound(ncols, nslices, sl), v1 = slice_bound(ncols, nslices, sl + 1);
 
@@ -113,9 +117,9 @@ k_bulk(Params p, int row0, int nrows, int gap0, int gap1, int nslices) {
         if (lane == 0) {
             int k = 0;
             for (int v = v0; v < v1; ++k) {
-                const int lim = (v < gap0) ? min(v1, gap0) : v1;
+                const int lim = (v < gapv) ? min(v1, gapv) : v1;
                 const int cnt = min(kColTile, lim - v);
-                const int a = (v < gap0) ? v : v + gap;
+                const int a = cbeg + ((v < gapv) ? v : v + gap);
                 const int s = k % kStages;
                 if (k >= kStages) mbar_wait(&empty_bar[s], ((k / kStages) - 1) & 1);
                 mbar_arrive_expect_tx(&full_bar[s], (uint32_t)cnt * 40u);
@@ -144,7 +148,7 @@ k_bulk(Params p, int row0, int nrows, int gap0, int gap1, int nslices) {
 
     int k = 0;
     for (int v = v0; v < v1; ++k) {
-        const int lim = (v < gap0) ? min(v1, gap0) : v1;
+        const int lim = (v < gapv) ? min(v1, gapv) : v1;
         const int cnt = min(kColTile, lim - v);
         const int s = k % kStages;
         mbar_wait(&full_bar[s], (k / kStages) & 1);
@@ -166,8 +170,8 @@ k_bulk(Params p, int row0, int nrows, int gap0, int gap1, int nslices) {
         v += cnt;
     }
     if (live) {
-        p.partA[(size_t)sl * p.chunk + r] = acc;
-        p.ovA[(size_t)sl * p.chunk + r] = ov;
+        p.partA[(size_t)(slot0 + sl) * p.chunk + r] = acc;
+        p.ovA[(size_t)(slot0 + sl) * p.chunk + r] = ov;
     }
 }
 
@@ -253,48 +257,124 @@ __global__ void __launch_bounds__(256) k_diag(Params p, int row0, int nrows) {
 // a3/a4: sequential resolution of one chunk (Alg. 4).
 // One CTA.  Warp 0 is the chain: lane l owns particle 32t+l of tile t; step j = lane j's
 // decision, published by __ballot_sync; lanes > j add their precomputed D(l,j) if j accepted.
-// Then all warps propagate the tile's accept mask to the rows of later tiles (block column
-// t of D), and the last warp prefetches the next diagonal block.
+// While the chain resolves tile t, the other warps (a) add the corrections of the previous
+// tile's accept mask A_{t-1} to the rows of tiles >= t+1 (block column t-1 of D, from L2) and
+// (b) stage what the chain needs for tile t+1 in shared memory: the diagonal block (t+1,t+1),
+// the block (t+1,t) -- applied by the chain warp itself as soon as A_t exists -- and the
+// per-row scalars.  One __syncthreads per tile.
 // accept iff no veto and l_B q_i sum + ln u < 0 (Eq. 1 in log form, strict; G3, G4).
 // ------------------------------------------------------------------------------------------
 constexpr int kChainThreads = 512;
 
+struct ChainTileStage {
+    double diag[kTile * kTile];   // D block (t, t)   [jj][lane]
+    double prev[kTile * kTile];   // D block (t, t-1) [jj][lane]
+    double lbq[kTile], lnu[kTile];
+    unsigned ovoD[kTile], ovnD[kTile];  // overlap words of the diagonal block
+    unsigned ovoP[kTile], ovnP[kTile];  // overlap words of block (t, t-1)
+};
+
+// Loads everything the chain needs for tile t into registers (issue phase) ...
+struct ChainStageRegs {
+    double d[5];
+    double sc;
+    unsigned w;
+};
+
+__device__ __forceinline__ void chain_stage_load(const Params& p, ChainStageRegs& rg, int row0, int t, int W,
+                                                 int idx, int nthreads) {
+    const double* dg = p.Dblk + (size_t)blk_index(t, t) * (kTile * kTile);
+    const double* pv = p.Dblk + (size_t)blk_index(t, t > 0 ? t - 1 : 0) * (kTile * kTile);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const int e = idx + k * nthreads;   // element of [diag | prev], 2048 in all
+        rg.d[k] = 0.0;
+        if (e < kTile * kTile) rg.d[k] = dg[e];
+        else if (e < 2 * kTile * kTile && t > 0) rg.d[k] = pv[e - kTile * kTile];
+    }
+    const int a = idx >> 5, l = idx & 31, r = t * kTile + l;
+    rg.sc = 0.0;
+    rg.w = 0u;
+    if (a == 0) rg.sc = p.lbq[row0 + r];
+    else if (a == 1) rg.sc = p.lnu[row0 + r];
+    else if (a == 2) rg.w = p.OVold[(size_t)r * W + t];
+    else if (a == 3) rg.w = p.OVnew[(size_t)r * W + t];
+    else if (a == 4 && t > 0) rg.w = p.OVold[(size_t)r * W + t - 1];
+    else if (a == 5 && t > 0) rg.w = p.OVnew[(size_t)r * W + t - 1];
+}
+
+// ... and writes them to the shared stage (after the loads have been issued).
+__device__ __forceinline__ void chain_stage_store(ChainTileStage& st, const ChainStageRegs& rg, int idx,
+                                                  int nthreads) {
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const int e = idx + k * nthreads;
+        if (e < kTile * kTile) st.diag[e] = rg.d[k];
+        else if (e < 2 * kTile * kTile) st.prev[e - kTile * kTile] = rg.d[k];
+    }
+    const int a = idx >> 5, l = idx & 31;
+    if (a == 0) st.lbq[l] = rg.sc;
+    else if (a == 1) st.lnu[l] = rg.sc;
+    else if (a == 2) st.ovoD[l] = rg.w;
+    else if (a == 3) st.ovnD[l] = rg.w;
+    else if (a == 4) st.ovoP[l] = rg.w;
+    else if (a == 5) st.ovnP[l] = rg.w;
+}
+
 __global__ void __launch_bounds__(kChainThreads, 1)
-k_chain(Params p, int row0, int nrows, int nslices, int last_chunk) {
+k_chain(Params p, int row0, int nrows, int nslots, int last_chunk) {
     __shared__ double sE[kChunkMax];
     __shared__ unsigned char sVeto[kChunkMax];
-    __shared__ double sDiag[2][kTile * kTile];      // diagonal D block of tile t (double buffered)
-    __shared__ double sLbq[2][kTile], sLnu[2][kTile];
-    __shared__ unsigned sOvo[2][kTile], sOvn[2][kTile];
-    __shared__ unsigned sA;
+    __shared__ ChainTileStage sT[2];
+    __shared__ unsigned sA[kChunkMax / kTile];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int nwarps = kChainThreads / 32;
     const int nt = nrows / kTile;
     const int W = p.chunk / kTile;
 
-    // prologue: reduce the partial sums in a fixed order
+    // prologue: reduce the partial sums in a fixed order (16 independent accumulators per row,
+    // combined in a fixed tree, so the result does not depend on scheduling)
     for (int r = tid; r < nrows; r += kChainThreads) {
-        double e = 0.0;
+        double e[16];
         int ov = 0;
-        for (int sl = 0; sl < nslices; ++sl) {
-            e += p.partA[(size_t)sl * p.chunk + r];
-            ov += p.ovA[(size_t)sl * p.chunk + r];
+#pragma unroll
+        for (int u = 0; u < 16; ++u) e[u] = 0.0;
+        for (int sl = 0; sl < nslots; sl += 16) {
+            double v[16];
+            int o[16];
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                const bool in = sl + u < nslots;
+                v[u] = in ? p.partA[(size_t)(sl + u) * p.chunk + r] : 0.0;
+                o[u] = in ? p.ovA[(size_t)(sl + u) * p.chunk + r] : 0;
+            }
+#pragma unroll
+            for (int u = 0; u < 16; ++u) { e[u] += v[u]; ov += o[u]; }
         }
-        for (int s = 0; s < nt; ++s) {
-            e += p.partD[(size_t)s * p.chunk + r];
-            ov += p.ovD[(size_t)s * p.chunk + r];
+        for (int s0 = 0; s0 < nt; s0 += 16) {
+            double v[16];
+            int o[16];
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                const bool in = s0 + u < nt;
+                v[u] = in ? p.partD[(size_t)(s0 + u) * p.chunk + r] : 0.0;
+                o[u] = in ? p.ovD[(size_t)(s0 + u) * p.chunk + r] : 0;
+            }
+#pragma unroll
+            for (int u = 0; u < 16; ++u) { e[u] += v[u]; ov += o[u]; }
         }
-        const int i = row0 + r;
-        sE[r] = e;
-        sVeto[r] = (unsigned char)(p.wall[i] | (ov > 0 ? kFlagOverlap : 0u));
+#pragma unroll
+        for (int w = 8; w > 0; w >>= 1)
+#pragma unroll
+            for (int u = 0; u < w; ++u) e[u] += e[u + w];
+        sE[r] = e[0];
+        sVeto[r] = (unsigned char)(p.wall[row0 + r] | (ov > 0 ? kFlagOverlap : 0u));
     }
-    for (int e = tid; e < kTile * kTile; e += kChainThreads) sDiag[0][e] = p.Dblk[e];
-    if (tid < kTile) {
-        sLbq[0][tid] = p.lbq[row0 + tid];
-        sLnu[0][tid] = p.lnu[row0 + tid];
-        sOvo[0][tid] = p.OVold[(size_t)tid * W];
-        sOvn[0][tid] = p.OVnew[(size_t)tid * W];
+    {
+        ChainStageRegs rg;
+        chain_stage_load(p, rg, row0, 0, W, tid, kChainThreads);
+        chain_stage_store(sT[0], rg, tid, kChainThreads);
     }
     __syncthreads();
 
@@ -303,19 +383,27 @@ k_chain(Params p, int row0, int nrows, int nslices, int last_chunk) {
 
     for (int t = 0; t < nt; ++t) {
         if (warp == 0) {
+            // ---------------- the chain ----------------
+            const ChainTileStage& st = sT[t & 1];
             const int r = t * kTile + lane, i = row0 + r;
-            const double* dg = sDiag[t & 1];
-            const double lbq = sLbq[t & 1][lane], lnu = sLnu[t & 1][lane];
+            const double lbq = st.lbq[lane], lnu = st.lnu[lane];
             double Eu = sE[r];
-            double Es = __fma_rn(lbq, Eu, lnu);
             const unsigned vflags = sVeto[r];
             const bool wallv = (vflags & kFlagWall) != 0u;
             bool ovv = (vflags & kFlagOverlap) != 0u;
-            const unsigned ovo = sOvo[t & 1][lane], ovn = sOvn[t & 1][lane];
+            if (t > 0) {  // corrections of the tile just resolved (block (t, t-1))
+                const unsigned Ap = sA[t - 1];
+#pragma unroll
+                for (int jj = 0; jj < kTile; ++jj)
+                    if ((Ap >> jj) & 1u) Eu = __dadd_rn(Eu, st.prev[jj * kTile + lane]);
+                ovv = ovv || (((st.ovnP[lane] & Ap) | (st.ovoP[lane] & ~Ap)) != 0u);
+            }
+            double Es = __fma_rn(lbq, Eu, lnu);
+            const unsigned ovo = st.ovoD[lane], ovn = st.ovnD[lane];
             unsigned A = 0u;
 #pragma unroll
             for (int j = 0; j < kTile; ++j) {
-                const double dj = dg[j * kTile + lane];       // 0 for lanes <= j
+                const double dj = st.diag[j * kTile + lane];   // 0 for lanes <= j
                 const double djs = __dmul_rn(lbq, dj);
                 const bool ok = !wallv && !ovv && (Es < 0.0);
                 const unsigned bal = __ballot_sync(0xffffffffu, ok);
@@ -327,6 +415,7 @@ k_chain(Params p, int row0, int nrows, int nslices, int last_chunk) {
                 }
                 ovv = ovv || ((((bit ? ovn : ovo) >> j) & 1u) != 0u);  // bits >= lane are 0
             }
+            if (lane == 0) sA[t] = A;
             const bool acc = ((A >> lane) & 1u) != 0u;
             const double dE = __dmul_rn(lbq, Eu);
             const bool tie = !wallv && !ovv && (fabs(Es) < 1e-8);
@@ -346,31 +435,43 @@ k_chain(Params p, int row0, int nrows, int nslices, int last_chunk) {
             n_wall += __popc(__ballot_sync(0xffffffffu, real && wallv));
             n_tie += __popc(__ballot_sync(0xffffffffu, real && tie));
             e_run += warp_sum(acc ? dE : 0.0);
-            if (lane == 0) sA = A;
-        }
-        __syncthreads();
-        const unsigned A = sA;
-        // propagate to later tiles: rows of tile t2 get sum over accepted jj of D(t2, t)[jj][lane]
-        for (int t2 = t + 1 + warp; t2 < nt; t2 += nwarps) {
-            const int r = t2 * kTile + lane;
-            const double* blk = p.Dblk + (size_t)blk_index(t2, t) * (kTile * kTile);
-            double e = sE[r];
-#pragma unroll 8
-            for (int jj = 0; jj < kTile; ++jj)
-                if ((A >> jj) & 1u) e = __dadd_rn(e, blk[jj * kTile + lane]);
-            sE[r] = e;
-            const unsigned on = p.OVnew[(size_t)r * W + t], oo = p.OVold[(size_t)r * W + t];
-            if (((on & A) | (oo & ~A)) != 0u) sVeto[r] |= (unsigned char)kFlagOverlap;
-        }
-        if (warp == nwarps - 1 && t + 1 < nt) {
-            const double* nb = p.Dblk + (size_t)blk_index(t + 1, t + 1) * (kTile * kTile);
-            double* dst = sDiag[(t + 1) & 1];
-            for (int e = lane; e < kTile * kTile; e += 32) dst[e] = nb[e];
-            const int rn = (t + 1) * kTile + lane;
-            sLbq[(t + 1) & 1][lane] = p.lbq[row0 + rn];
-            sLnu[(t + 1) & 1][lane] = p.lnu[row0 + rn];
-            sOvo[(t + 1) & 1][lane] = p.OVold[(size_t)rn * W + t + 1];
-            sOvn[(t + 1) & 1][lane] = p.OVnew[(size_t)rn * W + t + 1];
+        } else {
+            // ---------------- helpers ----------------
+            const int hid = tid - 32;
+            constexpr int nh = kChainThreads - 32;
+            const unsigned Ap = t > 0 ? sA[t - 1] : 0u;
+            // issue: corrections of mask A_{t-1} for the first far tile of this warp ...
+            int t2 = t + warp;   // tiles t+1 .. nt-1, round-robin over the helper warps
+            double v[kTile];
+            const bool far0 = t > 0 && t2 < nt;
+            {
+                const double* blk = p.Dblk + (size_t)blk_index(far0 ? t2 : 1, far0 ? t - 1 : 0) * (kTile * kTile);
+#pragma unroll
+                for (int jj = 0; jj < kTile; ++jj)
+                    v[jj] = (far0 && ((Ap >> jj) & 1u)) ? blk[jj * kTile + lane] : 0.0;
+            }
+            // ... and everything the chain needs for tile t+1
+            ChainStageRegs rg;
+            const bool stage = t + 1 < nt;
+            if (stage) chain_stage_load(p, rg, row0, t + 1, W, hid, nh);
+            if (stage) chain_stage_store(sT[(t + 1) & 1], rg, hid, nh);
+            // consume
+            bool first = true;
+            for (; t > 0 && t2 < nt; t2 += nwarps - 1) {
+                const int r = t2 * kTile + lane;
+                if (!first) {
+                    const double* blk = p.Dblk + (size_t)blk_index(t2, t - 1) * (kTile * kTile);
+#pragma unroll
+                    for (int jj = 0; jj < kTile; ++jj) v[jj] = ((Ap >> jj) & 1u) ? blk[jj * kTile + lane] : 0.0;
+                }
+                first = false;
+                const unsigned on = p.OVnew[(size_t)r * W + t - 1], oo = p.OVold[(size_t)r * W + t - 1];
+                double s4[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+                for (int jj = 0; jj < kTile; ++jj) s4[jj & 3] = __dadd_rn(s4[jj & 3], v[jj]);
+                sE[r] = __dadd_rn(sE[r], __dadd_rn(__dadd_rn(s4[0], s4[1]), __dadd_rn(s4[2], s4[3])));
+                if (((on & Ap) | (oo & ~Ap)) != 0u) sVeto[r] |= (unsigned char)kFlagOverlap;
+            }
         }
         __syncthreads();
     }

@@ -46,7 +46,7 @@ Layout make_layout(int64_t N) {
     const size_t nt = kChunkMax / kTile;
     L.xy = take(Np * 16); L.zq = take(Np * 16); L.hh = take(Np * 8); L.lbq = take(Np * 8);
     L.txy = take(Np * 16); L.tz = take(Np * 8); L.lnu = take(Np * 8); L.wall = take(Np);
-    L.partA = take((size_t)kMaxSlices * kChunkMax * 8); L.ovA = take((size_t)kMaxSlices * kChunkMax * 4);
+    L.partA = take((size_t)2 * kMaxSlices * kChunkMax * 8); L.ovA = take((size_t)2 * kMaxSlices * kChunkMax * 4);
     L.partD = take(nt * kChunkMax * 8); L.ovD = take(nt * kChunkMax * 4);
     L.Dblk = take(nt * (nt + 1) / 2 * kTile * kTile * 8);
     L.OVold = take((size_t)kChunkMax * nt * 4); L.OVnew = take((size_t)kChunkMax * nt * 4);
@@ -66,11 +66,13 @@ struct mc_handle {
     Layout L{};
     char* ws = nullptr;
     cudaStream_t stream = nullptr;
-    cudaStream_t cap_stream = nullptr;
+    cudaStream_t cap_stream = nullptr;   // graph capture origin (bulk kernels)
+    cudaStream_t cap_stream2 = nullptr;  // chain branch of the captured graph
+    cudaEvent_t ev_trial = nullptr, ev_bulk[2] = {nullptr, nullptr}, ev_chain[2] = {nullptr, nullptr};
     int num_sms = 148;
     int chunk = kChunkMax;
     bool use_graph = true;
-    bool overlap = false;
+    bool overlap = true;
     cudaGraphExec_t graph = nullptr;
     uint64_t launches = 0;
     uint64_t launches_per_sweep = 0;
@@ -91,39 +93,68 @@ void drop_graph(mc_handle* h) {
 
 int slices_for(const mc_handle* h, int nrows, int ncols) {
     const int rgs = (nrows + kBulkRowsPerCta - 1) / kBulkRowsPerCta;
-    int target = (2 * h->num_sms + rgs - 1) / rgs;      // two CTAs per SM
+    // two CTAs per SM, minus a few slots so that the chain CTA of the previous chunk (which runs
+    // concurrently on the other graph branch) always finds room on some SM
+    int target = (2 * h->num_sms - 4) / rgs;
     const int max_by_cols = ncols / 64 > 0 ? ncols / 64 : 1;  // at least 64 columns per slice
     if (target > max_by_cols) target = max_by_cols;
-    if (target > kMaxSlices) target = kMaxSlices;
+    if (target > kMaxSlices - 64) target = kMaxSlices - 64;
     if (target < 1) target = 1;
     return target;
 }
 
-// Enqueue one sweep on `s`.  Returns the number of kernels launched.
-int enqueue_sweep(mc_handle* h, cudaStream_t s, uint64_t* count) {
+// Enqueue one sweep.  sa carries k_trial and the bulk kernels, sb the per-chunk fix/diag/chain
+// kernels.  With sb == sa everything is serial; with two capturing streams (fork = true) the
+// chain of chunk c runs concurrently with the bulk kernel of chunk c+1:
+//   bulk(c)  : rows of chunk c x columns outside chunks c-1 and c      needs chain(c-2)
+//   fix(c)   : rows of chunk c x columns of chunk c-1 (final)          needs chain(c-1)
+//   diag(c)  : rows of chunk c x columns of chunk c                    needs chain(c-1) (buffers)
+//   chain(c) : needs bulk(c), fix(c), diag(c)
+// Both modes launch the same kernels with the same arguments, so results are bit-identical.
+int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uint64_t* count) {
     Params p = h->p;
     p.chunk = h->chunk;
     uint64_t n = 0;
-    k_trial<<<(p.Np + 255) / 256, 256, 0, s>>>(p);
+    k_trial<<<(p.Np + 255) / 256, 256, 0, sa>>>(p);
     ++n;
+    if (fork) {
+        cudaEventRecord(h->ev_trial, sa);
+        cudaStreamWaitEvent(sb, h->ev_trial, 0);
+    }
     const int nchunks = (p.Np + h->chunk - 1) / h->chunk;
     for (int c = 0; c < nchunks; ++c) {
         const int row0 = c * h->chunk;
         const int nrows = std::min(h->chunk, p.Np - row0);
-        const int ncols = p.Np - nrows;
-        int nslices = 0;
+        const int prev0 = c > 0 ? row0 - h->chunk : row0;   // start of chunk c-1 (== row0 for c == 0)
+        const int ncols = p.Np - (row0 + nrows - prev0);
+        Params pc = p;   // partial buffers alternate with the chunk parity
+        pc.partA = p.partA + (size_t)(c & 1) * kMaxSlices * kChunkMax;
+        pc.ovA = p.ovA + (size_t)(c & 1) * kMaxSlices * kChunkMax;
+        const int rgs = (nrows + kBulkRowsPerCta - 1) / kBulkRowsPerCta;
+        int nslA = 0, nslF = 0;
+        if (fork && c >= 2) cudaStreamWaitEvent(sa, h->ev_chain[c & 1], 0);
         if (ncols > 0) {
-            nslices = slices_for(h, nrows, ncols);
-            dim3 grid((nrows + kBulkRowsPerCta - 1) / kBulkRowsPerCta, nslices);
-            k_bulk<<<grid, kBulkRowsPerCta + 32, 0, s>>>(p, row0, nrows, row0, row0 + nrows, nslices);
+            nslA = slices_for(h, nrows, ncols);
+            k_bulk<<<dim3(rgs, nslA), kBulkRowsPerCta + 32, 0, sa>>>(pc, row0, nrows, 0, p.Np, prev0, row0 + nrows,
+                                                                     nslA, 0);
+            ++n;
+        }
+        if (fork) cudaEventRecord(h->ev_bulk[c & 1], sa);
+        if (c > 0) {
+            nslF = std::max(1, std::min(32, (row0 - prev0) / 32));
+            k_bulk<<<dim3(rgs, nslF), kBulkRowsPerCta + 32, 0, sb>>>(pc, row0, nrows, prev0, row0, row0, row0, nslF,
+                                                                     nslA);
             ++n;
         }
         const int nt = nrows / kTile;
-        k_diag<<<(nt * nt + 7) / 8, 256, 0, s>>>(p, row0, nrows);
+        k_diag<<<(nt * nt + 7) / 8, 256, 0, sb>>>(pc, row0, nrows);
         ++n;
-        k_chain<<<1, kChainThreads, 0, s>>>(p, row0, nrows, nslices, c == nchunks - 1 ? 1 : 0);
+        if (fork) cudaStreamWaitEvent(sb, h->ev_bulk[c & 1], 0);
+        k_chain<<<1, kChainThreads, 0, sb>>>(pc, row0, nrows, nslA + nslF, c == nchunks - 1 ? 1 : 0);
         ++n;
+        if (fork) cudaEventRecord(h->ev_chain[c & 1], sb);
     }
+    if (fork) cudaStreamWaitEvent(sa, h->ev_chain[(nchunks - 1) & 1], 0);   // join
     if (count) *count = n;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(MC_ECUDA, std::string("sweep launch: ") + cudaGetErrorString(e));
@@ -133,11 +164,20 @@ int enqueue_sweep(mc_handle* h, cudaStream_t s, uint64_t* count) {
 int build_graph(mc_handle* h) {
     drop_graph(h);
     cudaGraph_t g = nullptr;
-    // capture on a private stream (the caller's may be the legacy default stream, which cannot capture)
-    if (!h->cap_stream) CUDA_TRY(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    // capture on private streams (the caller's may be the legacy default stream, which cannot capture)
+    if (!h->cap_stream) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&h->cap_stream2, cudaStreamNonBlocking));
+        CUDA_TRY(cudaEventCreateWithFlags(&h->ev_trial, cudaEventDisableTiming));
+        for (int k = 0; k < 2; ++k) {
+            CUDA_TRY(cudaEventCreateWithFlags(&h->ev_bulk[k], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&h->ev_chain[k], cudaEventDisableTiming));
+        }
+    }
     CUDA_TRY(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
     uint64_t n = 0;
-    const int rc = enqueue_sweep(h, h->cap_stream, &n);
+    const int rc = h->overlap ? enqueue_sweep(h, h->cap_stream, h->cap_stream2, true, &n)
+                              : enqueue_sweep(h, h->cap_stream, h->cap_stream, false, &n);
     cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
     if (rc != MC_OK) {
         if (g) cudaGraphDestroy(g);
@@ -243,7 +283,12 @@ int mc_free(mc_handle* h) {
     if (!h) return MC_OK;
     cudaStreamSynchronize(h->stream);
     drop_graph(h);
-    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    if (h->cap_stream) {
+        cudaStreamDestroy(h->cap_stream);
+        cudaStreamDestroy(h->cap_stream2);
+        cudaEventDestroy(h->ev_trial);
+        for (int k = 0; k < 2; ++k) { cudaEventDestroy(h->ev_bulk[k]); cudaEventDestroy(h->ev_chain[k]); }
+    }
     delete h;
     return MC_OK;
 }
@@ -261,7 +306,7 @@ int mc_sweep(mc_handle* h, int64_t n) {
     } else {
         for (int64_t s = 0; s < n; ++s) {
             uint64_t c = 0;
-            const int rc = enqueue_sweep(h, h->stream, &c);
+            const int rc = enqueue_sweep(h, h->stream, h->stream, false, &c);
             if (rc != MC_OK) return rc;
             h->launches += c;
         }
