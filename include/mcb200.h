@@ -77,6 +77,9 @@ int mc_sweep(mc_handle* h, int64_t n);
  * during warm-up).  Synchronises. */
 int mc_energy(mc_handle* h, double* E_host);
 
+/* Same energy, left in device memory (E_dev, one double); enqueued, no host sync. */
+int mc_energy_dev(mc_handle* h, double* E_dev);
+
 /* Adds the current configuration's ordered-pair distance counts into caller-owned device
  * accumulators: hist_dev [2][2][nbins] and n_centres_dev [2] (uint64).  Species index 0 if
  * q > 0 else 1.  Centres are ions with |x_i| <= centre_rmax (bulk only); partners
@@ -110,6 +113,20 @@ const char* mc_last_error(void);
  * `millis` ms on the given stream and returns FP64 FMA warp-lane instructions per second
  * (thread-level DFMA/s).  Synchronises.  Not part of the hot path. */
 int mc_measure_fp64_peak(void* stream, double millis, double* dfma_per_second_host);
+
+/* Diagnostics for the roofline: runs ONE sweep (it advances the chain exactly as mc_sweep(h, 1)
+ * does, same kernels, same arguments, bit-identical result) with the kernels launched one after
+ * the other on the handle's stream and a CUDA event pair around every launch.  Fills
+ * ms_host[MC_NKERNELS] with the summed device time per kernel class and launches_host[MC_NKERNELS]
+ * with the launch counts, pairs_host[MC_NKERNELS] with the pair evaluations (counted towards
+ * N(N-1): rows x columns, no speculative work) each class covered.  Synchronises. */
+#define MC_K_TRIAL 0
+#define MC_K_BULK 1   /* rows of a chunk x columns outside chunks c-1, c                  */
+#define MC_K_FIX 2    /* rows of a chunk x columns of chunk c-1 (same kernel as MC_K_BULK) */
+#define MC_K_DIAG 3   /* rows of a chunk x columns of the chunk, with speculation          */
+#define MC_K_CHAIN 4  /* sequential resolution                                             */
+#define MC_NKERNELS 5
+int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_t* pairs_host);
 
 /* Tuning knobs (diagnostic; defaults are right for B200): key "chunk" = rows resolved per
  * chain kernel (multiple of 32, 32..1024), "graph" = 0/1 use CUDA graphs, "overlap" = 0/1 run

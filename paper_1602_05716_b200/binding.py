@@ -19,7 +19,8 @@ MC_OK, MC_EINVAL, MC_EOVERLAP, MC_EOUTSIDE, MC_ENOSPACE, MC_ECUDA = 0, -1, -2, -
 _CODES = {-1: "MC_EINVAL", -2: "MC_EOVERLAP", -3: "MC_EOUTSIDE", -4: "MC_ENOSPACE", -5: "MC_ECUDA"}
 
 EXPORTS = (
-    "mc_workspace_bytes", "mc_init", "mc_sweep", "mc_energy", "mc_pair_hist", "mc_sweep_host",
+    "mc_workspace_bytes", "mc_init", "mc_sweep", "mc_energy", "mc_energy_dev", "mc_pair_hist", "mc_sweep_host",
+    "mc_sweep_timed",
     "mc_get_positions", "mc_set_positions", "mc_get_sweep_index", "mc_set_sweep_index", "mc_get_stats",
     "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option",
     "mc_get_launch_count",
@@ -54,6 +55,8 @@ def load_library() -> C.CDLL:
     lib.mc_init.argtypes = [C.POINTER(vp), i64, vp, vp, vp, dbl, dbl, dbl, u64, vp, C.c_size_t, vp, C.c_int]
     lib.mc_sweep.argtypes = [vp, i64]
     lib.mc_energy.argtypes = [vp, C.POINTER(dbl)]
+    lib.mc_energy_dev.argtypes = [vp, vp]
+    lib.mc_sweep_timed.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64), C.POINTER(i64)]
     lib.mc_pair_hist.argtypes = [vp, dbl, C.c_int, dbl, vp, vp]
     lib.mc_sweep_host.argtypes = [vp, i64, vp, vp, C.POINTER(mc_stats)]
     lib.mc_get_positions.argtypes = [vp, vp]
@@ -152,6 +155,22 @@ class MCSystem:
         return e.value
 
     energy = mc_energy
+
+    def mc_energy_dev(self, out=None) -> torch.Tensor:
+        if out is None:
+            out = torch.empty(1, dtype=torch.float64, device=self.device)
+        assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 1
+        _check(self._lib.mc_energy_dev(self._h, out.data_ptr()))
+        return out
+
+    KERNEL_CLASSES = ("k_trial", "k_bulk", "k_bulk(fix)", "k_diag", "k_chain")
+
+    def mc_sweep_timed(self) -> dict:
+        """One sweep with an event pair around every launch: {class: (ms, launches, pair evals)}."""
+        n = len(self.KERNEL_CLASSES)
+        ms, cnt, pairs = (C.c_double * n)(), (C.c_int64 * n)(), (C.c_int64 * n)()
+        _check(self._lib.mc_sweep_timed(self._h, ms, cnt, pairs))
+        return {k: (ms[i], cnt[i], pairs[i]) for i, k in enumerate(self.KERNEL_CLASSES)}
 
     def mc_pair_hist(self, bin_width, nbins, centre_rmax, hist=None, n_centres=None):
         if hist is None:

@@ -103,6 +103,20 @@ int slices_for(const mc_handle* h, int nrows, int ncols) {
     return target;
 }
 
+// Optional per-launch timing (mc_sweep_timed): an event pair around every launch, serial mode only.
+struct SweepTimer {
+    std::vector<cudaEvent_t> ev;   // 2 per launch
+    std::vector<int> kind;
+    int64_t pairs[MC_NKERNELS] = {0, 0, 0, 0, 0};
+    void before(cudaStream_t s, int k) {
+        cudaEvent_t a, b;
+        cudaEventCreate(&a); cudaEventCreate(&b);
+        ev.push_back(a); ev.push_back(b); kind.push_back(k);
+        cudaEventRecord(a, s);
+    }
+    void after(cudaStream_t s) { cudaEventRecord(ev.back(), s); }
+};
+
 // Enqueue one sweep.  sa carries k_trial and the bulk kernels, sb the per-chunk fix/diag/chain
 // kernels.  With sb == sa everything is serial; with two capturing streams (fork = true) the
 // chain of chunk c runs concurrently with the bulk kernel of chunk c+1:
@@ -111,11 +125,14 @@ int slices_for(const mc_handle* h, int nrows, int ncols) {
 //   diag(c)  : rows of chunk c x columns of chunk c                    needs chain(c-1) (buffers)
 //   chain(c) : needs bulk(c), fix(c), diag(c)
 // Both modes launch the same kernels with the same arguments, so results are bit-identical.
-int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uint64_t* count) {
+int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uint64_t* count,
+                  SweepTimer* tm = nullptr) {
     Params p = h->p;
     p.chunk = h->chunk;
     uint64_t n = 0;
+    if (tm) tm->before(sa, MC_K_TRIAL);
     k_trial<<<(p.Np + 255) / 256, 256, 0, sa>>>(p);
+    if (tm) tm->after(sa);
     ++n;
     if (fork) {
         cudaEventRecord(h->ev_trial, sa);
@@ -127,6 +144,7 @@ int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uin
         const int nrows = std::min(h->chunk, p.Np - row0);
         const int prev0 = c > 0 ? row0 - h->chunk : row0;   // start of chunk c-1 (== row0 for c == 0)
         const int ncols = p.Np - (row0 + nrows - prev0);
+        const int64_t real_rows = std::max(0, std::min(nrows, p.N - row0));
         Params pc = p;   // partial buffers alternate with the chunk parity
         pc.partA = p.partA + (size_t)(c & 1) * kMaxSlices * kChunkMax;
         pc.ovA = p.ovA + (size_t)(c & 1) * kMaxSlices * kChunkMax;
@@ -135,22 +153,39 @@ int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uin
         if (fork && c >= 2) cudaStreamWaitEvent(sa, h->ev_chain[c & 1], 0);
         if (ncols > 0) {
             nslA = slices_for(h, nrows, ncols);
+            if (tm) {
+                tm->before(sa, MC_K_BULK);
+                tm->pairs[MC_K_BULK] += real_rows * (int64_t)(p.N - std::min(p.N, row0 + nrows) + prev0);
+            }
             k_bulk<<<dim3(rgs, nslA), kBulkRowsPerCta + 32, 0, sa>>>(pc, row0, nrows, 0, p.Np, prev0, row0 + nrows,
                                                                      nslA, 0);
+            if (tm) tm->after(sa);
             ++n;
         }
         if (fork) cudaEventRecord(h->ev_bulk[c & 1], sa);
         if (c > 0) {
             nslF = std::max(1, std::min(32, (row0 - prev0) / 32));
+            if (tm) {
+                tm->before(sb, MC_K_FIX);
+                tm->pairs[MC_K_FIX] += real_rows * (int64_t)(row0 - prev0);
+            }
             k_bulk<<<dim3(rgs, nslF), kBulkRowsPerCta + 32, 0, sb>>>(pc, row0, nrows, prev0, row0, row0, row0, nslF,
                                                                      nslA);
+            if (tm) tm->after(sb);
             ++n;
         }
         const int nt = nrows / kTile;
+        if (tm) {
+            tm->before(sb, MC_K_DIAG);
+            tm->pairs[MC_K_DIAG] += real_rows * (real_rows - 1);
+        }
         k_diag<<<(nt * nt + 7) / 8, 256, 0, sb>>>(pc, row0, nrows);
+        if (tm) tm->after(sb);
         ++n;
         if (fork) cudaStreamWaitEvent(sb, h->ev_bulk[c & 1], 0);
+        if (tm) tm->before(sb, MC_K_CHAIN);
         k_chain<<<1, kChainThreads, 0, sb>>>(pc, row0, nrows, nslA + nslF, c == nchunks - 1 ? 1 : 0);
+        if (tm) tm->after(sb);
         ++n;
         if (fork) cudaEventRecord(h->ev_chain[c & 1], sb);
     }
@@ -321,6 +356,31 @@ int mc_energy(mc_handle* h, double* E_host) {
     if (rc != MC_OK) return rc;
     CUDA_TRY(cudaMemcpyAsync(E_host, out, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return MC_OK;
+}
+
+int mc_energy_dev(mc_handle* h, double* E_dev) {
+    if (!h || !E_dev) return fail(MC_EINVAL, "null argument");
+    return enqueue_energy(h, E_dev, 0, 0);
+}
+
+int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_t* pairs_host) {
+    if (!h || !ms_host || !launches_host || !pairs_host) return fail(MC_EINVAL, "null argument");
+    SweepTimer tm;
+    uint64_t c = 0;
+    const int rc = enqueue_sweep(h, h->stream, h->stream, false, &c, &tm);
+    h->launches += c;
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    for (int k = 0; k < MC_NKERNELS; ++k) { ms_host[k] = 0.0; launches_host[k] = 0; pairs_host[k] = tm.pairs[k]; }
+    for (size_t i = 0; i < tm.kind.size(); ++i) {
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, tm.ev[2 * i], tm.ev[2 * i + 1]);
+        ms_host[tm.kind[i]] += ms;
+        launches_host[tm.kind[i]] += 1;
+    }
+    for (cudaEvent_t ev : tm.ev) cudaEventDestroy(ev);
+    if (rc != MC_OK) return rc;
+    if (e != cudaSuccess) return fail(MC_ECUDA, std::string("mc_sweep_timed: ") + cudaGetErrorString(e));
     return MC_OK;
 }
 
