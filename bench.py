@@ -125,23 +125,33 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------
 # the reference arm: the CPU oracle, as it stands, on the host cores
 # ---------------------------------------------------------------------------------------------------
-def oracle_sample_rate(w, threads: int, seconds: float, first: int = 0):
-    """Pair evaluations per second of oracle trials first.. of sweep 0 (bounded sample), and the sample."""
+def oracle_sample_rate(w, threads: int, seconds: float, state=None):
+    """Pair evaluations per second of the oracle on a bounded sample: consecutive trials (in sweep order,
+    continuing into the next sweeps) for about ``seconds``.  Returns (rate, trials done, seconds, state)."""
     from oracle import Oracle
-    pos, q, d = w.arrays()
-    o = Oracle(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, w.seed, validate=False, threads=threads)
-    k = min(w.N - first, 64)
-    t0 = time.perf_counter()
-    o.partial_sweep(first, k)
-    dt = time.perf_counter() - t0
-    done, spent = k, dt
-    want = int(min(w.N - first - done, max(0, (seconds - dt) / max(dt / k, 1e-9))))
-    if want > 0:
+    if state is None:
+        pos, q, d = w.arrays()
+        state = {"o": Oracle(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, w.seed, validate=False, threads=threads),
+                 "next": 0}
+        state["o"].partial_sweep(0, min(8, w.N))          # thread start-up, untimed
+        state["next"] = min(8, w.N) % w.N
+    o = state["o"]
+    done, spent, batch = 0, 0.0, 32
+    while spent < seconds:
+        first = state["next"]
+        cnt = min(batch, w.N - first)
         t0 = time.perf_counter()
-        o.partial_sweep(first + done, want)
-        spent += time.perf_counter() - t0
-        done += want
-    return done * (w.N - 1) / spent, done, spent
+        o.partial_sweep(first, cnt)
+        dt = time.perf_counter() - t0
+        spent += dt
+        done += cnt
+        state["next"] = first + cnt
+        if state["next"] >= w.N:                          # next sweep of the same chain
+            o.sweep_index = o.sweep_index + 1
+            state["next"] = 0
+        if dt < 0.25 * seconds:
+            batch = min(w.N, max(batch, int(batch * min(8.0, 0.25 * seconds / max(dt, 1e-6)))))
+    return done * (w.N - 1) / spent, done, spent, state
 
 
 def run_reference(args, w):
@@ -149,20 +159,18 @@ def run_reference(args, w):
     if rank != 0:
         return 0
     cores = os.cpu_count() or 1
-    per_step = max(0.5, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
-    first = 0
+    per_step = max(0.5, min(15.0, 150.0 / max(1, args.steps + args.warmup)))
+    state = None
     for _ in range(args.warmup):
-        _, n, _ = oracle_sample_rate(w, cores, per_step, first)
-        first = (first + n) % max(1, w.N - 4096)
+        _, _, _, state = oracle_sample_rate(w, cores, per_step, state)
     tot_pairs, tot_s, trials = 0.0, 0.0, 0
     for _ in range(args.steps):
-        r, n, s = oracle_sample_rate(w, cores, per_step, first)
+        r, n, s, state = oracle_sample_rate(w, cores, per_step, state)
         tot_pairs += r * s
         tot_s += s
         trials += n
-        first = (first + n) % max(1, w.N - 4096)
     value = tot_pairs / tot_s
-    sample = (f"{trials} consecutive trials of sweep 0 in {args.steps} steps (~{per_step:.1f} s each), "
+    sample = (f"{trials} consecutive trials in sweep order in {args.steps} steps (~{per_step:.1f} s each), "
               f"each trial against all N-1 partners, OpenMP over j")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps,
@@ -323,14 +331,17 @@ def run_ours(args, w):
     step_frac = value / world * FP64_INSTR_PER_PAIR / peak_instr
 
     # ---- CPU baseline: the oracle as it stands, bounded sample, this box's cores ----
-    cores = os.cpu_count() or 1
-    cpu_all, n_all, s_all = oracle_sample_rate(w, cores, 12.0)
-    cpu_one, n_one, s_one = oracle_sample_rate(w, 1, 8.0)
-    cpu_baseline = {"value": cpu_all, "unit": UNIT, "cores": cores, "kind": "oracle",
-                    "sample": f"first {n_all} trials of sweep 0 at N={N} ({s_all:.1f} s, OpenMP over j, {cores} threads)",
-                    "single_thread": {"value": cpu_one, "cores": 1,
-                                      "sample": f"first {n_one} trials of sweep 0 ({s_one:.1f} s)"},
-                    "paper_context": "paper: 440x over one Xeon core on Tesla K20 (PAPER.md:315)"}
+    cpu_baseline = None
+    if not args.skip_cpu_baseline:
+        cores = os.cpu_count() or 1
+        cpu_all, n_all, s_all, _ = oracle_sample_rate(w, cores, 12.0)
+        cpu_one, n_one, s_one, _ = oracle_sample_rate(w, 1, 8.0)
+        cpu_baseline = {"value": cpu_all, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": (f"{n_all} consecutive trials in sweep order from sweep 0 at N={N} ({s_all:.1f} s, "
+                                   f"OpenMP over j, {cores} threads)"),
+                        "single_thread": {"value": cpu_one, "cores": 1,
+                                          "sample": f"first {n_one} trials of sweep 0 ({s_one:.1f} s)"},
+                        "paper_context": "paper: 440x over one Xeon core on Tesla K20 (PAPER.md:315)"}
 
     st = sysm.mc_get_stats()
     line = {
@@ -363,6 +374,8 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default=None, help="workloads.CONFIGS name (default: the N=65536 headline)")
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--skip-cpu-baseline", action="store_true",
+                    help="leave out the oracle timing (profiling runs under ncu only)")
     args = ap.parse_args(argv)
     from paper_1602_05716_b200 import workloads as W
     w = W.by_name(args.workload) if args.workload else W.HEADLINE

@@ -130,7 +130,11 @@ int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_
 
 /* Tuning knobs (diagnostic; defaults are right for B200): key "chunk" = rows resolved per
  * chain kernel (multiple of 32, 32..1024), "graph" = 0/1 use CUDA graphs, "overlap" = 0/1 run
- * the chain concurrently with the next chunk's bulk kernel.  Returns MC_EINVAL for unknown keys. */
+ * the chain concurrently with the next chunk's bulk kernel, "bulk_rows" = 1|2 rows per thread of
+ * the bulk kernel, "bulk_ctas" = 1..4 bulk CTAs per SM the grid is sized for, "uniform_path" =
+ * 0/1 allow the equal-diameter specialisation.  Every setting gives the same accept/reject
+ * sequence; settings that change the partition of a row's sum change dE by rounding only.
+ * Returns MC_EINVAL for unknown keys. */
 int mc_set_option(mc_handle* h, const char* key, int64_t value);
 
 /* Number of kernels this handle launched (or replayed through graphs) since mc_init. */

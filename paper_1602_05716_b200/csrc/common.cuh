@@ -10,7 +10,7 @@ constexpr int kTile = 32;            // chain tile: one warp lane per particle
 constexpr int kChunkMax = 1024;      // rows resolved by one chain kernel (max)
 constexpr int kColTile = 128;        // columns staged per bulk-copy stage
 constexpr int kStages = 4;           // smem ring depth of the bulk kernel
-constexpr int kBulkRowsPerCta = 256; // consumer threads (= rows) per bulk CTA
+constexpr int kBulkThreads = 256;    // consumer threads per bulk CTA (each owns 1 or 2 rows)
 constexpr int kMaxSlices = 512;      // upper bound on column slices of the bulk kernel
 constexpr double kGhostCoord = 1.0e9;
 constexpr double kGhostStep = 1.0e6;
@@ -22,8 +22,8 @@ struct DevState {
     unsigned long long sweep;
     unsigned long long accepted, veto_overlap, veto_wall, near_ties;
     double E_run;
-    int err;   // validation result (0 ok, MC_E* otherwise)
-    int pad;
+    int err;        // validation result (0 ok, MC_E* otherwise)
+    int d_differs;  // set by k_check_particles if not all diameters are equal
 };
 
 // ---------------------------------------------------------------------------------------------

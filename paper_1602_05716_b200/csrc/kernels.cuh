@@ -83,18 +83,43 @@ struct __align__(16) ColStage {
     double h[kColTile];
 };
 
+// slice boundaries in the virtual column space: multiples of 8, so that every staged segment
+// holds a multiple of 8 columns (gap and range boundaries are multiples of 32) and the inner
+// loop needs no tail
 __device__ __forceinline__ int slice_bound(int ncols, int nslices, int sl) {
-    return (int)(((long long)(ncols >> 1) * sl) / nslices) << 1;  // even boundaries
+    return (int)(((long long)(ncols >> 3) * sl) / nslices) << 3;
 }
 
-__global__ void __launch_bounds__(kBulkRowsPerCta + 32, 2)
+// One pair evaluation (Eq. 2; Alg. 2): 26 FP64-pipe instructions
+// (24 if UNIFORM: s2 = d^2 precomputed) + 2 MUFU.RSQ64H.  The overlap test r2n < s2 compares the
+// bit patterns as integers (both are non-negative doubles, so the order is the same) to keep
+// the DSETP off the FP64 pipe; ovacc collects the sign bits.
+template <bool UNIFORM>
+__device__ __forceinline__ void pair_eval(double xi, double yi, double zi, double txi, double tyi, double tzi,
+                                          double hi, double s2u, const double2 a, const double2 b, double hj,
+                                          double& acc, int& ovacc) {
+    const double r2o = dist2(__dadd_rn(xi, -a.x), __dadd_rn(yi, -a.y), __dadd_rn(zi, -b.x));
+    const double r2n = dist2(__dadd_rn(txi, -a.x), __dadd_rn(tyi, -a.y), __dadd_rn(tzi, -b.x));
+    double s2 = s2u;
+    if (!UNIFORM) {
+        const double sij = __dadd_rn(hi, hj);
+        s2 = __dmul_rn(sij, sij);
+    }
+    ovacc |= (int)((__double_as_longlong(r2n) - __double_as_longlong(s2)) >> 32);   // sign bit <=> r2n < s2
+    const double du = __dadd_rn(rsqrt_fast(r2n), -rsqrt_fast(r2o));
+    acc = __fma_rn(b.y, du, acc);
+}
+
+template <int ROWS, bool UNIFORM>
+__global__ void __launch_bounds__(kBulkThreads + 32, ROWS == 1 ? 4 : 2)
 k_bulk(Params p, int row0, int nrows, int cbeg, int cend, int gap0, int gap1, int nslices, int slot0) {
     __shared__ ColStage stage[kStages];
     __shared__ __align__(8) uint64_t full_bar[kStages];
     __shared__ __align__(8) uint64_t empty_bar[kStages];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    constexpr int kConsumerWarps = kBulkRowsPerCta / 32;
+    constexpr int kConsumerWarps = kBulkThreads / 32;
+    constexpr int kRowsPerCta = kBulkThreads * ROWS;
     // columns = [cbeg, cend) minus [gap0, gap1) (gap inside the range, or empty), as a virtual
     // index space v in [0, ncols): actual column = cbeg + v (+ gap if at or past the gap)
     const int gap = gap1 - gap0;
@@ -122,29 +147,34 @@ k_bulk(Params p, int row0, int nrows, int cbeg, int cend, int gap0, int gap1, in
                 const int a = cbeg + ((v < gapv) ? v : v + gap);
                 const int s = k % kStages;
                 if (k >= kStages) mbar_wait(&empty_bar[s], ((k / kStages) - 1) & 1);
-                mbar_arrive_expect_tx(&full_bar[s], (uint32_t)cnt * 40u);
+                mbar_arrive_expect_tx(&full_bar[s], (uint32_t)cnt * (UNIFORM ? 32u : 40u));
                 bulk_g2s(stage[s].xy, p.xy + a, (uint32_t)cnt * 16u, &full_bar[s]);
                 bulk_g2s(stage[s].zq, p.zq + a, (uint32_t)cnt * 16u, &full_bar[s]);
-                bulk_g2s(stage[s].h, p.hh + a, (uint32_t)cnt * 8u, &full_bar[s]);
+                if (!UNIFORM) bulk_g2s(stage[s].h, p.hh + a, (uint32_t)cnt * 8u, &full_bar[s]);
                 v += cnt;
             }
         }
         return;
     }
 
-    // ---- consumers: one row per thread ----
-    const int r = blockIdx.x * kBulkRowsPerCta + tid;  // row within the chunk
-    const bool live = r < nrows;
-    const bool warp_live = blockIdx.x * kBulkRowsPerCta + warp * 32 < nrows;  // whole warp past the chunk
-    const int i = row0 + (live ? r : 0);
-    const double2 xyi = p.xy[i];
-    const double2 zqi = p.zq[i];
-    const double2 txyi = p.txy[i];
-    const double xi = xyi.x, yi = xyi.y, zi = zqi.x;
-    const double txi = txyi.x, tyi = txyi.y, tzi = p.tz[i];
-    const double hi = p.hh[i];
-    double acc = 0.0;
-    int ov = 0;
+    // ---- consumers: ROWS rows per thread (row r, r + kBulkThreads, ...) ----
+    const int rbase = blockIdx.x * kRowsPerCta;
+    const bool warp_live = rbase + warp * 32 < nrows;   // whole warp past the chunk: only feed the barriers
+    double xi[ROWS], yi[ROWS], zi[ROWS], txi[ROWS], tyi[ROWS], tzi[ROWS], hi[ROWS], acc[ROWS];
+    int ov[ROWS];
+#pragma unroll
+    for (int u = 0; u < ROWS; ++u) {
+        const int r = rbase + u * kBulkThreads + tid;
+        const int i = row0 + (r < nrows ? r : 0);
+        const double2 xyi = p.xy[i];
+        const double2 txyi = p.txy[i];
+        xi[u] = xyi.x; yi[u] = xyi.y; zi[u] = p.zq[i].x;
+        txi[u] = txyi.x; tyi[u] = txyi.y; tzi[u] = p.tz[i];
+        hi[u] = p.hh[i];
+        acc[u] = 0.0;
+        ov[u] = 0;
+    }
+    const double s2u = __dmul_rn(__dadd_rn(hi[0], hi[0]), __dadd_rn(hi[0], hi[0]));   // UNIFORM: (h + h)^2
 
     int k = 0;
     for (int v = v0; v < v1; ++k) {
@@ -153,25 +183,31 @@ k_bulk(Params p, int row0, int nrows, int cbeg, int cend, int gap0, int gap1, in
         const int s = k % kStages;
         mbar_wait(&full_bar[s], (k / kStages) & 1);
         const ColStage& st = stage[s];
-#pragma unroll 4
-        for (int j = 0; j < (warp_live ? cnt : 0); ++j) {
-            const double2 a = st.xy[j];
-            const double2 b = st.zq[j];
-            const double hj = st.h[j];
-            const double r2o = dist2(__dadd_rn(xi, -a.x), __dadd_rn(yi, -a.y), __dadd_rn(zi, -b.x));
-            const double r2n = dist2(__dadd_rn(txi, -a.x), __dadd_rn(tyi, -a.y), __dadd_rn(tzi, -b.x));
-            const double sij = __dadd_rn(hi, hj);
-            ov += (r2n < __dmul_rn(sij, sij)) ? 1 : 0;
-            const double du = __dadd_rn(rsqrt_fast(r2n), -rsqrt_fast(r2o));
-            acc = __fma_rn(b.y, du, acc);
+        if (warp_live) {
+            for (int j0 = 0; j0 < cnt; j0 += 4) {     // cnt is a multiple of 8
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    const double2 a = st.xy[j0 + jj];
+                    const double2 b = st.zq[j0 + jj];
+                    const double hj = UNIFORM ? 0.0 : st.h[j0 + jj];
+#pragma unroll
+                    for (int u = 0; u < ROWS; ++u)
+                        pair_eval<UNIFORM>(xi[u], yi[u], zi[u], txi[u], tyi[u], tzi[u], hi[u], s2u, a, b, hj, acc[u],
+                                           ov[u]);
+                }
+            }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty_bar[s]);
         v += cnt;
     }
-    if (live) {
-        p.partA[(size_t)(slot0 + sl) * p.chunk + r] = acc;
-        p.ovA[(size_t)(slot0 + sl) * p.chunk + r] = ov;
+#pragma unroll
+    for (int u = 0; u < ROWS; ++u) {
+        const int r = rbase + u * kBulkThreads + tid;
+        if (r < nrows) {
+            p.partA[(size_t)(slot0 + sl) * p.chunk + r] = acc[u];
+            p.ovA[(size_t)(slot0 + sl) * p.chunk + r] = ov[u] < 0 ? 1 : 0;
+        }
     }
 }
 
@@ -543,6 +579,7 @@ __global__ void k_check_particles(Params p, const double* d) {
         if (!(a >= 0.0) || dist2(xy.x, xy.y, zq.x) > __dmul_rn(a, a)) err = -3;
     }
     if (err) atomicMin(&p.st->err, err == -1 ? -1000 : err);  // EINVAL outranks the others
+    if (di != d[0]) p.st->d_differs = 1;
 }
 
 // ------------------------------------------------------------------------------------------

@@ -73,6 +73,11 @@ struct mc_handle {
     int chunk = kChunkMax;
     bool use_graph = true;
     bool overlap = true;
+    int bulk_rows = 1;       // rows per consumer thread of k_bulk (1 or 2)
+    int bulk_ctas = 2;       // k_bulk CTAs per SM the grid is sized for
+    bool uniform_d = false;  // all diameters equal: s_ij^2 is one constant
+    bool allow_uniform = true;
+    bool all_d_equal = false;
     cudaGraphExec_t graph = nullptr;
     uint64_t launches = 0;
     uint64_t launches_per_sweep = 0;
@@ -91,16 +96,33 @@ void drop_graph(mc_handle* h) {
     }
 }
 
+int bulk_row_groups(const mc_handle* h, int nrows) {
+    const int per = kBulkThreads * h->bulk_rows;
+    return (nrows + per - 1) / per;
+}
+
 int slices_for(const mc_handle* h, int nrows, int ncols) {
-    const int rgs = (nrows + kBulkRowsPerCta - 1) / kBulkRowsPerCta;
-    // two CTAs per SM, minus a few slots so that the chain CTA of the previous chunk (which runs
-    // concurrently on the other graph branch) always finds room on some SM
-    int target = (2 * h->num_sms - 4) / rgs;
+    const int rgs = bulk_row_groups(h, nrows);
+    // bulk_ctas CTAs per SM on all SMs but one: the chain CTA of the previous chunk (which runs
+    // concurrently on the other graph branch) needs a whole SM's registers
+    int target = (h->bulk_ctas * (h->num_sms - 1)) / rgs;
     const int max_by_cols = ncols / 64 > 0 ? ncols / 64 : 1;  // at least 64 columns per slice
     if (target > max_by_cols) target = max_by_cols;
     if (target > kMaxSlices - 64) target = kMaxSlices - 64;
     if (target < 1) target = 1;
     return target;
+}
+
+void launch_bulk(const mc_handle* h, cudaStream_t s, const Params& pc, int row0, int nrows, int cbeg, int cend,
+                 int gap0, int gap1, int nsl, int slot0) {
+    const dim3 grid(bulk_row_groups(h, nrows), nsl), block(kBulkThreads + 32);
+    if (h->bulk_rows == 2) {
+        if (h->uniform_d) k_bulk<2, true><<<grid, block, 0, s>>>(pc, row0, nrows, cbeg, cend, gap0, gap1, nsl, slot0);
+        else k_bulk<2, false><<<grid, block, 0, s>>>(pc, row0, nrows, cbeg, cend, gap0, gap1, nsl, slot0);
+    } else {
+        if (h->uniform_d) k_bulk<1, true><<<grid, block, 0, s>>>(pc, row0, nrows, cbeg, cend, gap0, gap1, nsl, slot0);
+        else k_bulk<1, false><<<grid, block, 0, s>>>(pc, row0, nrows, cbeg, cend, gap0, gap1, nsl, slot0);
+    }
 }
 
 // Optional per-launch timing (mc_sweep_timed): an event pair around every launch, serial mode only.
@@ -148,7 +170,6 @@ int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uin
         Params pc = p;   // partial buffers alternate with the chunk parity
         pc.partA = p.partA + (size_t)(c & 1) * kMaxSlices * kChunkMax;
         pc.ovA = p.ovA + (size_t)(c & 1) * kMaxSlices * kChunkMax;
-        const int rgs = (nrows + kBulkRowsPerCta - 1) / kBulkRowsPerCta;
         int nslA = 0, nslF = 0;
         if (fork && c >= 2) cudaStreamWaitEvent(sa, h->ev_chain[c & 1], 0);
         if (ncols > 0) {
@@ -157,8 +178,7 @@ int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uin
                 tm->before(sa, MC_K_BULK);
                 tm->pairs[MC_K_BULK] += real_rows * (int64_t)(p.N - std::min(p.N, row0 + nrows) + prev0);
             }
-            k_bulk<<<dim3(rgs, nslA), kBulkRowsPerCta + 32, 0, sa>>>(pc, row0, nrows, 0, p.Np, prev0, row0 + nrows,
-                                                                     nslA, 0);
+            launch_bulk(h, sa, pc, row0, nrows, 0, p.Np, prev0, row0 + nrows, nslA, 0);
             if (tm) tm->after(sa);
             ++n;
         }
@@ -169,8 +189,7 @@ int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uin
                 tm->before(sb, MC_K_FIX);
                 tm->pairs[MC_K_FIX] += real_rows * (int64_t)(row0 - prev0);
             }
-            k_bulk<<<dim3(rgs, nslF), kBulkRowsPerCta + 32, 0, sb>>>(pc, row0, nrows, prev0, row0, row0, row0, nslF,
-                                                                     nslA);
+            launch_bulk(h, sb, pc, row0, nrows, prev0, row0, row0, row0, nslF, nslA);
             if (tm) tm->after(sb);
             ++n;
         }
@@ -305,6 +324,8 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     e = cudaMemcpyAsync(&st, p.st, sizeof(st), cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return bail(fail(MC_ECUDA, std::string("init: ") + cudaGetErrorString(e)));
+    h->all_d_equal = st.d_differs == 0;
+    h->uniform_d = h->allow_uniform && h->all_d_equal;
     if (st.err != 0) {
         if (st.err <= -1000) return bail(fail(MC_EINVAL, "non-finite input or diameter <= 0"));
         if (st.err == -3) return bail(fail(MC_EOUTSIDE, "an ion sticks out of the cavity"));
@@ -519,6 +540,15 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
         h->use_graph = value != 0;
     } else if (!std::strcmp(key, "overlap")) {
         h->overlap = value != 0;
+    } else if (!std::strcmp(key, "bulk_rows")) {
+        if (value != 1 && value != 2) return fail(MC_EINVAL, "bulk_rows must be 1 or 2");
+        h->bulk_rows = (int)value;
+    } else if (!std::strcmp(key, "bulk_ctas")) {
+        if (value < 1 || value > 4) return fail(MC_EINVAL, "bulk_ctas must be in 1..4");
+        h->bulk_ctas = (int)value;
+    } else if (!std::strcmp(key, "uniform_path")) {
+        h->allow_uniform = value != 0;
+        h->uniform_d = h->allow_uniform && h->all_d_equal;
     } else {
         return fail(MC_EINVAL, std::string("unknown option ") + key);
     }

@@ -51,12 +51,13 @@ def test_library_is_sm100a_native_with_bulk_async_copies(lib):
     from paper_1602_05716_b200 import binding
     out = subprocess.run(["cuobjdump", "-lelf", str(binding._LIBPATH)], capture_output=True, text=True).stdout
     assert "sm_100a" in out
-    sass = subprocess.run(["cuobjdump", "-sass", "-fun", "_ZN3mcb6k_bulkENS_6ParamsEiiiiiiii",
-                           str(binding._LIBPATH)], capture_output=True, text=True).stdout
-    if sass.strip():
-        assert "UBLKCP" in sass          # cp.async.bulk (TMA unit) staging
-        assert "MUFU.RSQ64H" in sass     # FP64 rsqrt seed
-        assert "DFMA" in sass
+    sass = subprocess.run(["cuobjdump", "-sass", str(binding._LIBPATH)], capture_output=True, text=True).stdout
+    bulk = [blk for blk in sass.split("Function :")[1:] if "k_bulk" in blk.splitlines()[0]]
+    assert bulk, "no k_bulk instantiation in the SASS"
+    for blk in bulk:
+        assert "UBLKCP" in blk          # cp.async.bulk (TMA unit) staging
+        assert "MUFU.RSQ64H" in blk     # FP64 rsqrt seed
+        assert "DFMA" in blk
 
 
 def test_host_argument_checks_need_no_gpu(lib):
