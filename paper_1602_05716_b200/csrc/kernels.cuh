@@ -90,24 +90,58 @@ __device__ __forceinline__ int slice_bound(int ncols, int nslices, int sl) {
     return (int)(((long long)(ncols >> 3) * sl) / nslices) << 3;
 }
 
-// One pair evaluation (Eq. 2; Alg. 2): 26 FP64-pipe instructions
-// (24 if UNIFORM: s2 = d^2 precomputed) + 2 MUFU.RSQ64H.  The overlap test r2n < s2 compares the
-// bit patterns as integers (both are non-negative doubles, so the order is the same) to keep
-// the DSETP off the FP64 pipe; ovacc collects the sign bits.
+// One pair evaluation (Eq. 2; Alg. 2): 22 FP64-pipe instructions
+// (24 if diameters differ) + 2 MUFU.RSQ64H.
+//   dx = x_i - x_j ...            3 DADD          r2o = fma(dz,dz,fma(dy,dy,dx dx))   3
+//   w  = 2 D.(x_i - x_j) + |D|^2  3 DFMA          r2n = r2o + w                       1
+//   (D = x~_i - x_i: |x~_i - x_j|^2 = |x_i - x_j|^2 + 2 D.(x_i - x_j) + |D|^2)
+//   2 x rsqrt refinement          10              du, acc                             2
+// The overlap veto is an integer test off the FP64 pipe: the running minimum of
+// the high word of r2n (minus the high word of s_ij^2 if diameters differ).  r2n here is not in
+// the evaluation order reading G11 fixes for the veto, so a row whose minimum falls within
+// kOvBand high-word steps (2^-16 relative) of the threshold is re-examined exactly by
+// recheck_overlap(); everything outside the band is decided by the minimum alone.
+constexpr int kOvBand = 16;
+
+struct RowRegs {
+    double x, y, z;     // current position of the row's particle
+    double ex, ey, ez;  // 2 (x~ - x)
+    double c;           // |x~ - x|^2
+    double h;           // d/2
+    double acc;
+    int m;              // running minimum of the overlap key
+};
+
 template <bool UNIFORM>
-__device__ __forceinline__ void pair_eval(double xi, double yi, double zi, double txi, double tyi, double tzi,
-                                          double hi, double s2u, const double2 a, const double2 b, double hj,
-                                          double& acc, int& ovacc) {
-    const double r2o = dist2(__dadd_rn(xi, -a.x), __dadd_rn(yi, -a.y), __dadd_rn(zi, -b.x));
-    const double r2n = dist2(__dadd_rn(txi, -a.x), __dadd_rn(tyi, -a.y), __dadd_rn(tzi, -b.x));
-    double s2 = s2u;
+__device__ __forceinline__ int pair_eval(RowRegs& r, const double2 a, const double2 b, double hj) {
+    const double dx = __dadd_rn(r.x, -a.x), dy = __dadd_rn(r.y, -a.y), dz = __dadd_rn(r.z, -b.x);
+    const double r2o = dist2(dx, dy, dz);
+    const double w = __fma_rn(r.ex, dx, __fma_rn(r.ey, dy, __fma_rn(r.ez, dz, r.c)));
+    const double r2n = __dadd_rn(r2o, w);
+    int key = __double2hiint(r2n);
     if (!UNIFORM) {
-        const double sij = __dadd_rn(hi, hj);
-        s2 = __dmul_rn(sij, sij);
+        const double sij = __dadd_rn(r.h, hj);
+        key -= __double2hiint(__dmul_rn(sij, sij));
     }
-    ovacc |= (int)((__double_as_longlong(r2n) - __double_as_longlong(s2)) >> 32);   // sign bit <=> r2n < s2
     const double du = __dadd_rn(rsqrt_fast(r2n), -rsqrt_fast(r2o));
-    acc = __fma_rn(b.y, du, acc);
+    r.acc = __fma_rn(b.y, du, r.acc);
+    return key;
+}
+
+// Exact overlap test of trial i against the columns [v0, v1) of the virtual column space
+// (reading G7/G11: r2 = fma(dz,dz,fma(dy,dy,dx dx)) of the rounded differences, strict <).
+__device__ __noinline__ int recheck_overlap(const double2* xy, const double2* zq, const double* hh, double2 t,
+                                            double tz, double hi, int v0, int v1, int cbeg, int gapv, int gap) {
+    int ov = 0;
+    for (int v = v0; v < v1; ++v) {
+        const int j = cbeg + (v < gapv ? v : v + gap);
+        const double2 a = xy[j];
+        const double zj = zq[j].x;
+        const double sij = __dadd_rn(hi, hh[j]);
+        const double r2n = dist2(__dadd_rn(t.x, -a.x), __dadd_rn(t.y, -a.y), __dadd_rn(tz, -zj));
+        ov |= (r2n < __dmul_rn(sij, sij)) ? 1 : 0;
+    }
+    return ov;
 }
 
 template <int ROWS, bool UNIFORM>
@@ -160,21 +194,21 @@ k_bulk(Params p, int row0, int nrows, int cbeg, int cend, int gap0, int gap1, in
     // ---- consumers: ROWS rows per thread (row r, r + kBulkThreads, ...) ----
     const int rbase = blockIdx.x * kRowsPerCta;
     const bool warp_live = rbase + warp * 32 < nrows;   // whole warp past the chunk: only feed the barriers
-    double xi[ROWS], yi[ROWS], zi[ROWS], txi[ROWS], tyi[ROWS], tzi[ROWS], hi[ROWS], acc[ROWS];
-    int ov[ROWS];
+    RowRegs R[ROWS];
 #pragma unroll
     for (int u = 0; u < ROWS; ++u) {
         const int r = rbase + u * kBulkThreads + tid;
         const int i = row0 + (r < nrows ? r : 0);
         const double2 xyi = p.xy[i];
         const double2 txyi = p.txy[i];
-        xi[u] = xyi.x; yi[u] = xyi.y; zi[u] = p.zq[i].x;
-        txi[u] = txyi.x; tyi[u] = txyi.y; tzi[u] = p.tz[i];
-        hi[u] = p.hh[i];
-        acc[u] = 0.0;
-        ov[u] = 0;
+        R[u].x = xyi.x; R[u].y = xyi.y; R[u].z = p.zq[i].x;
+        const double Dx = __dadd_rn(txyi.x, -xyi.x), Dy = __dadd_rn(txyi.y, -xyi.y), Dz = __dadd_rn(p.tz[i], -R[u].z);
+        R[u].ex = __dadd_rn(Dx, Dx); R[u].ey = __dadd_rn(Dy, Dy); R[u].ez = __dadd_rn(Dz, Dz);
+        R[u].c = dist2(Dx, Dy, Dz);
+        R[u].h = p.hh[i];
+        R[u].acc = 0.0;
+        R[u].m = 0x7fffffff;
     }
-    const double s2u = __dmul_rn(__dadd_rn(hi[0], hi[0]), __dadd_rn(hi[0], hi[0]));   // UNIFORM: (h + h)^2
 
     int k = 0;
     for (int v = v0; v < v1; ++k) {
@@ -184,16 +218,19 @@ k_bulk(Params p, int row0, int nrows, int cbeg, int cend, int gap0, int gap1, in
         mbar_wait(&full_bar[s], (k / kStages) & 1);
         const ColStage& st = stage[s];
         if (warp_live) {
+#pragma unroll 1
             for (int j0 = 0; j0 < cnt; j0 += 4) {     // cnt is a multiple of 8
 #pragma unroll
-                for (int jj = 0; jj < 4; ++jj) {
-                    const double2 a = st.xy[j0 + jj];
-                    const double2 b = st.zq[j0 + jj];
-                    const double hj = UNIFORM ? 0.0 : st.h[j0 + jj];
+                for (int jj = 0; jj < 4; jj += 2) {
+                    const double2 a0 = st.xy[j0 + jj], a1 = st.xy[j0 + jj + 1];
+                    const double2 b0 = st.zq[j0 + jj], b1 = st.zq[j0 + jj + 1];
+                    const double h0 = UNIFORM ? 0.0 : st.h[j0 + jj], h1 = UNIFORM ? 0.0 : st.h[j0 + jj + 1];
 #pragma unroll
-                    for (int u = 0; u < ROWS; ++u)
-                        pair_eval<UNIFORM>(xi[u], yi[u], zi[u], txi[u], tyi[u], tzi[u], hi[u], s2u, a, b, hj, acc[u],
-                                           ov[u]);
+                    for (int u = 0; u < ROWS; ++u) {
+                        const int k0 = pair_eval<UNIFORM>(R[u], a0, b0, h0);
+                        const int k1 = pair_eval<UNIFORM>(R[u], a1, b1, h1);
+                        R[u].m = __vimin3_s32(R[u].m, k0, k1);
+                    }
                 }
             }
         }
@@ -204,9 +241,18 @@ k_bulk(Params p, int row0, int nrows, int cbeg, int cend, int gap0, int gap1, in
 #pragma unroll
     for (int u = 0; u < ROWS; ++u) {
         const int r = rbase + u * kBulkThreads + tid;
+        // overlap key: high word of r2n relative to the high word of s^2
+        int key = R[u].m;
+        if (UNIFORM) {
+            const double s = __dadd_rn(R[u].h, R[u].h);
+            key -= __double2hiint(__dmul_rn(s, s));
+        }
+        int ov = key < 0 ? 1 : 0;
+        if (r < nrows && key >= -kOvBand && key <= kOvBand)
+            ov = recheck_overlap(p.xy, p.zq, p.hh, p.txy[row0 + r], p.tz[row0 + r], R[u].h, v0, v1, cbeg, gapv, gap);
         if (r < nrows) {
-            p.partA[(size_t)(slot0 + sl) * p.chunk + r] = acc[u];
-            p.ovA[(size_t)(slot0 + sl) * p.chunk + r] = ov[u] < 0 ? 1 : 0;
+            p.partA[(size_t)(slot0 + sl) * p.chunk + r] = R[u].acc;
+            p.ovA[(size_t)(slot0 + sl) * p.chunk + r] = ov;
         }
     }
 }
