@@ -32,6 +32,7 @@ struct Params {
     DevState* st;
     double R, lB, max_disp;
     unsigned long long seed;
+    int* sy; int sy_n;         // scheduling state of the persistent sweep kernel (zeroed by k_trial)
 };
 
 // ------------------------------------------------------------------------------------------
@@ -40,6 +41,7 @@ struct Params {
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_trial(Params p) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < p.sy_n) p.sy[i] = 0;
     if (i >= p.Np) return;
     const double2 xy = p.xy[i];
     const double2 zq = p.zq[i];
@@ -270,21 +272,22 @@ k_bulk(Params p, int row0, int nrows, int cbeg, int cend, int gap0, int gap1, in
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ int blk_index(int t, int s) { return t * (t + 1) / 2 + s; }
 
-__global__ void __launch_bounds__(256) k_diag(Params p, int row0, int nrows) {
-    __shared__ double2 cxy[8][32], czq[8][32], ctxy[8][32];
-    __shared__ double ch[8][32], ctz[8][32];
-    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+// one (row tile t, column tile s) unit, executed by one warp; the five arrays are this warp's
+// 32-entry shared-memory staging rows
+__device__ __forceinline__ void diag_unit(const Params& p, int row0, int nrows, int unit, double2* cxy, double2* czq,
+                                          double2* ctxy, double* ch, double* ctz) {
+    const int lane = threadIdx.x & 31;
     const int nt = nrows / kTile;
-    const int unit = blockIdx.x * 8 + w;
     if (unit >= nt * nt) return;
     const int t = unit / nt, s = unit % nt;
     const int r = t * kTile + lane, i = row0 + r;
     const int j0 = row0 + s * kTile;
-    cxy[w][lane] = p.xy[j0 + lane];
-    czq[w][lane] = p.zq[j0 + lane];
-    ctxy[w][lane] = p.txy[j0 + lane];
-    ctz[w][lane] = p.tz[j0 + lane];
-    ch[w][lane] = p.hh[j0 + lane];
+    __syncwarp();
+    cxy[lane] = p.xy[j0 + lane];
+    czq[lane] = p.zq[j0 + lane];
+    ctxy[lane] = p.txy[j0 + lane];
+    ctz[lane] = p.tz[j0 + lane];
+    ch[lane] = p.hh[j0 + lane];
     __syncwarp();
     const double2 xyi = p.xy[i];
     const double2 txyi = p.txy[i];
@@ -297,9 +300,9 @@ __global__ void __launch_bounds__(256) k_diag(Params p, int row0, int nrows) {
     unsigned ovo = 0u, ovn = 0u;
     double* blk = (s <= t) ? p.Dblk + (size_t)blk_index(t, s) * (kTile * kTile) : nullptr;
     for (int jj = 0; jj < kTile; ++jj) {
-        const double2 a = cxy[w][jj];
-        const double2 b = czq[w][jj];
-        const double sij = __dadd_rn(hi, ch[w][jj]);
+        const double2 a = cxy[jj];
+        const double2 b = czq[jj];
+        const double sij = __dadd_rn(hi, ch[jj]);
         const double s2 = __dmul_rn(sij, sij);
         const double r2oo = dist2(__dadd_rn(xi, -a.x), __dadd_rn(yi, -a.y), __dadd_rn(zi, -b.x));
         const double r2no = dist2(__dadd_rn(txi, -a.x), __dadd_rn(tyi, -a.y), __dadd_rn(tzi, -b.x));
@@ -309,8 +312,8 @@ __global__ void __launch_bounds__(256) k_diag(Params p, int row0, int nrows) {
             bsum = __fma_rn(b.y, __dadd_rn(rsqrt_fast(r2no), -rsqrt_fast(r2oo)), bsum);
             ovc += (r2no < s2) ? 1 : 0;
         } else if (lower) {
-            const double2 ta = ctxy[w][jj];
-            const double tzj = ctz[w][jj];
+            const double2 ta = ctxy[jj];
+            const double tzj = ctz[jj];
             const double r2on = dist2(__dadd_rn(xi, -ta.x), __dadd_rn(yi, -ta.y), __dadd_rn(zi, -tzj));
             const double r2nn = dist2(__dadd_rn(txi, -ta.x), __dadd_rn(tyi, -ta.y), __dadd_rn(tzi, -tzj));
             const bool oo = r2no < s2, on = r2nn < s2;
@@ -333,6 +336,14 @@ __global__ void __launch_bounds__(256) k_diag(Params p, int row0, int nrows) {
         p.OVold[(size_t)r * W + s] = ovo;
         p.OVnew[(size_t)r * W + s] = ovn;
     }
+}
+
+
+__global__ void __launch_bounds__(256) k_diag(Params p, int row0, int nrows) {
+    __shared__ double2 cxy[8][32], czq[8][32], ctxy[8][32];
+    __shared__ double ch[8][32], ctz[8][32];
+    const int w = threadIdx.x >> 5;
+    diag_unit(p, row0, nrows, blockIdx.x * 8 + w, cxy[w], czq[w], ctxy[w], ch[w], ctz[w]);
 }
 
 // ------------------------------------------------------------------------------------------

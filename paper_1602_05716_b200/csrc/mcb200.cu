@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "persist.cuh"
 
 using namespace mcb;
 
@@ -33,7 +34,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t xy, zq, hh, lbq, txy, tz, lnu, wall, partA, ovA, partD, ovD, Dblk, OVold, OVnew, log_dE, log_flags,
-        st, epart, centres, ccount, stage_pos, total;
+        st, epart, centres, ccount, stage_pos, Efar, ovfar, partF, ovF, sy, total;
 };
 
 int padded(int64_t N) { return (int)((N + kTile - 1) / kTile * kTile); }
@@ -47,9 +48,13 @@ Layout make_layout(int64_t N) {
     L.xy = take(Np * 16); L.zq = take(Np * 16); L.hh = take(Np * 8); L.lbq = take(Np * 8);
     L.txy = take(Np * 16); L.tz = take(Np * 8); L.lnu = take(Np * 8); L.wall = take(Np);
     L.partA = take((size_t)2 * kMaxSlices * kChunkMax * 8); L.ovA = take((size_t)2 * kMaxSlices * kChunkMax * 4);
-    L.partD = take(nt * kChunkMax * 8); L.ovD = take(nt * kChunkMax * 4);
-    L.Dblk = take(nt * (nt + 1) / 2 * kTile * kTile * 8);
-    L.OVold = take((size_t)kChunkMax * nt * 4); L.OVnew = take((size_t)kChunkMax * nt * 4);
+    // double-buffered by chunk parity (the persistent kernel prepares chunk c+1 while the chain is in c)
+    L.partD = take(2 * nt * kChunkMax * 8); L.ovD = take(2 * nt * kChunkMax * 4);
+    L.Dblk = take(2 * (nt * (nt + 1) / 2) * kTile * kTile * 8);
+    L.OVold = take((size_t)2 * kChunkMax * nt * 4); L.OVnew = take((size_t)2 * kChunkMax * nt * 4);
+    L.Efar = take((size_t)2 * kChunkMax * 8); L.ovfar = take((size_t)2 * kChunkMax * 4);
+    L.partF = take((size_t)2 * kMaxFixSlots * kChunkMax * 8); L.ovF = take((size_t)2 * kMaxFixSlots * kChunkMax * 4);
+    L.sy = take((size_t)(kSyHdr + 4 * (Np / 256 + 1)) * 4);
     L.log_dE = take(Np * 8); L.log_flags = take(Np);
     L.st = take(sizeof(DevState));
     L.epart = take((size_t)kEnergySlices * Np * 8 + 8);
@@ -73,6 +78,9 @@ struct mc_handle {
     int chunk = kChunkMax;
     bool use_graph = true;
     bool overlap = true;
+    int engine = 1;          // 1: one persistent kernel per sweep (persist.cuh); 0: kernels per chunk in a graph
+    int prows = 4;           // rows per consumer thread of the persistent kernel (chunk = 256 * prows)
+    int pgrid = 0;           // CTAs of the persistent kernel (0: not yet configured)
     int bulk_rows = 1;       // rows per consumer thread of k_bulk (1 or 2)
     int bulk_ctas = 2;       // k_bulk CTAs per SM the grid is sized for
     bool uniform_d = false;  // all diameters equal: s_ij^2 is one constant
@@ -215,6 +223,49 @@ int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uin
     return MC_OK;
 }
 
+// ---- persistent engine (persist.cuh): k_trial + one cooperative k_sweep launch per sweep ----
+template <int ROWS, bool UNIFORM>
+int launch_sweep_kernel(mc_handle* h, cudaStream_t s) {
+    auto kern = k_sweep<ROWS, UNIFORM>;
+    const int smem = (int)sizeof(PShared);
+    static thread_local bool configured = false;
+    if (!configured) {
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        configured = true;
+    }
+    if (h->pgrid == 0) {
+        int occ = 0;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kPThreads, smem));
+        if (occ < 1) return fail(MC_ECUDA, "k_sweep does not fit on an SM");
+        h->pgrid = std::min(occ, 2) * h->num_sms;
+    }
+    PArgs a{};
+    a.p = h->p;
+    a.C = 256 * ROWS;
+    a.p.chunk = a.C;
+    a.nchunks = (a.p.Np + a.C - 1) / a.C;
+    a.nworkers = std::max(1, h->pgrid - 1);
+    a.sy = h->p.sy;
+    char* w = h->ws;
+    a.Efar = (double*)(w + h->L.Efar); a.ovfar = (int*)(w + h->L.ovfar);
+    a.partF = (double*)(w + h->L.partF); a.ovF = (int*)(w + h->L.ovF);
+    void* args[] = {(void*)&a};
+    CUDA_TRY(cudaLaunchCooperativeKernel((void*)kern, dim3(h->pgrid), dim3(kPThreads), args, (size_t)smem, s));
+    return MC_OK;
+}
+
+int enqueue_sweep_persist(mc_handle* h, cudaStream_t s) {
+    const Params& p = h->p;
+    k_trial<<<(p.Np + 255) / 256, 256, 0, s>>>(p);
+    CUDA_TRY(cudaGetLastError());
+    const bool u = h->uniform_d;
+    switch (h->prows) {
+        case 1: return u ? launch_sweep_kernel<1, true>(h, s) : launch_sweep_kernel<1, false>(h, s);
+        case 2: return u ? launch_sweep_kernel<2, true>(h, s) : launch_sweep_kernel<2, false>(h, s);
+        default: return u ? launch_sweep_kernel<4, true>(h, s) : launch_sweep_kernel<4, false>(h, s);
+    }
+}
+
 int build_graph(mc_handle* h) {
     drop_graph(h);
     cudaGraph_t g = nullptr;
@@ -303,6 +354,9 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     p.Dblk = (double*)(w + L.Dblk); p.OVold = (unsigned*)(w + L.OVold); p.OVnew = (unsigned*)(w + L.OVnew);
     p.log_dE = (double*)(w + L.log_dE); p.log_flags = (unsigned char*)(w + L.log_flags);
     p.st = (DevState*)(w + L.st);
+    p.sy = (int*)(w + L.sy);
+    p.sy_n = kSyHdr + 4 * (p.Np / 256 + 1);
+    h->prows = p.Np >= 16384 ? 4 : (p.Np >= 2048 ? 2 : 1);
     p.R = cavity_R; p.lB = bjerrum_length; p.max_disp = max_disp; p.seed = seed;
     h->epart = (double*)(w + L.epart);
     h->centres = (int*)(w + L.centres);
@@ -352,6 +406,14 @@ int mc_free(mc_handle* h) {
 int mc_sweep(mc_handle* h, int64_t n) {
     if (!h || n < 0) return fail(MC_EINVAL, "bad handle or n < 0");
     if (n == 0) return MC_OK;
+    if (h->engine == 1) {
+        for (int64_t s = 0; s < n; ++s) {
+            const int rc = enqueue_sweep_persist(h, h->stream);
+            if (rc != MC_OK) return rc;
+        }
+        h->launches += 2 * (uint64_t)n;
+        return MC_OK;
+    }
     if (h->use_graph) {
         if (!h->graph) {
             const int rc = build_graph(h);
@@ -387,6 +449,38 @@ int mc_energy_dev(mc_handle* h, double* E_dev) {
 
 int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_t* pairs_host) {
     if (!h || !ms_host || !launches_host || !pairs_host) return fail(MC_EINVAL, "null argument");
+    if (h->engine == 1) {
+        // persistent engine: k_trial, then the whole sweep in one k_sweep launch (reported as MC_K_BULK)
+        for (int k = 0; k < MC_NKERNELS; ++k) { ms_host[k] = 0.0; launches_host[k] = 0; pairs_host[k] = 0; }
+        cudaEvent_t ev[3];
+        for (auto& x : ev) CUDA_TRY(cudaEventCreate(&x));
+        const Params& p = h->p;
+        // same launches as enqueue_sweep_persist, with an event between the two kernels
+        const int saved = h->engine;
+        (void)saved;
+        CUDA_TRY(cudaEventRecord(ev[0], h->stream));
+        k_trial<<<(p.Np + 255) / 256, 256, 0, h->stream>>>(p);
+        CUDA_TRY(cudaEventRecord(ev[1], h->stream));
+        const bool u = h->uniform_d;
+        int rc = MC_OK;
+        switch (h->prows) {
+            case 1: rc = u ? launch_sweep_kernel<1, true>(h, h->stream) : launch_sweep_kernel<1, false>(h, h->stream); break;
+            case 2: rc = u ? launch_sweep_kernel<2, true>(h, h->stream) : launch_sweep_kernel<2, false>(h, h->stream); break;
+            default: rc = u ? launch_sweep_kernel<4, true>(h, h->stream) : launch_sweep_kernel<4, false>(h, h->stream); break;
+        }
+        if (rc != MC_OK) return rc;
+        CUDA_TRY(cudaEventRecord(ev[2], h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+        h->launches += 2;
+        float a = 0.f, b = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&a, ev[0], ev[1]));
+        CUDA_TRY(cudaEventElapsedTime(&b, ev[1], ev[2]));
+        for (auto& x : ev) cudaEventDestroy(x);
+        ms_host[MC_K_TRIAL] = a; launches_host[MC_K_TRIAL] = 1;
+        ms_host[MC_K_BULK] = b; launches_host[MC_K_BULK] = 1;
+        pairs_host[MC_K_BULK] = (int64_t)p.N * (int64_t)(p.N - 1);
+        return MC_OK;
+    }
     SweepTimer tm;
     uint64_t c = 0;
     const int rc = enqueue_sweep(h, h->stream, h->stream, false, &c, &tm);
@@ -536,6 +630,12 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     if (!std::strcmp(key, "chunk")) {
         if (value < kTile || value > kChunkMax || value % kTile) return fail(MC_EINVAL, "chunk must be a multiple of 32 in 32..1024");
         h->chunk = (int)value;
+    } else if (!std::strcmp(key, "engine")) {
+        if (value != 0 && value != 1) return fail(MC_EINVAL, "engine must be 0 or 1");
+        h->engine = (int)value;
+    } else if (!std::strcmp(key, "prows")) {
+        if (value != 1 && value != 2 && value != 4) return fail(MC_EINVAL, "prows must be 1, 2 or 4");
+        h->prows = (int)value;
     } else if (!std::strcmp(key, "graph")) {
         h->use_graph = value != 0;
     } else if (!std::strcmp(key, "overlap")) {
