@@ -128,6 +128,13 @@ int mc_measure_fp64_peak(void* stream, double millis, double* dfma_per_second_ho
 #define MC_NKERNELS 5
 int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_t* pairs_host);
 
+/* Diagnostics of the persistent sweep kernel (option "debug" = 1): SM-clock cycle counters of the
+ * last sweep, out16_host[16]: [0] chain warp, whole sweep; [1] of which waiting for the first tile
+ * of a chunk; [2] waiting for later tiles; [3] helper 0 waiting for FAR/DIAG of a chunk; [4] for
+ * FIX; [5] summed cycles worker CTAs spent fetching items; [6..9] number of exit/DIAG/FAR/FIX
+ * items fetched.  Synchronises. */
+int mc_debug_counters(mc_handle* h, int64_t* out16_host);
+
 /* Tuning knobs (diagnostic; defaults are right for B200): key "chunk" = rows resolved per
  * chain kernel (multiple of 32, 32..1024), "graph" = 0/1 use CUDA graphs, "overlap" = 0/1 run
  * the chain concurrently with the next chunk's bulk kernel, "bulk_rows" = 1|2 rows per thread of

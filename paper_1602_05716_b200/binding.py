@@ -22,7 +22,7 @@ EXPORTS = (
     "mc_workspace_bytes", "mc_init", "mc_sweep", "mc_energy", "mc_energy_dev", "mc_pair_hist", "mc_sweep_host",
     "mc_sweep_timed",
     "mc_get_positions", "mc_set_positions", "mc_get_sweep_index", "mc_set_sweep_index", "mc_get_stats",
-    "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option",
+    "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option", "mc_debug_counters",
     "mc_get_launch_count",
 )
 
@@ -70,6 +70,7 @@ def load_library() -> C.CDLL:
     lib.mc_measure_fp64_peak.argtypes = [vp, dbl, C.POINTER(dbl)]
     lib.mc_set_option.argtypes = [vp, C.c_char_p, i64]
     lib.mc_get_launch_count.argtypes = [vp, C.POINTER(u64)]
+    lib.mc_debug_counters.argtypes = [vp, C.POINTER(C.c_int64)]
     for name in EXPORTS:
         if name not in ("mc_workspace_bytes", "mc_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -244,6 +245,11 @@ class MCSystem:
 
     def mc_set_option(self, key: str, value: int):
         _check(self._lib.mc_set_option(self._h, key.encode(), int(value)))
+
+    def mc_debug_counters(self) -> list:
+        out = (C.c_int64 * 16)()
+        _check(self._lib.mc_debug_counters(self._h, out))
+        return list(out)
 
     def mc_get_launch_count(self) -> int:
         n = C.c_uint64()

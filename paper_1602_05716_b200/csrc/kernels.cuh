@@ -33,7 +33,24 @@ struct Params {
     double R, lB, max_disp;
     unsigned long long seed;
     int* sy; int sy_n;         // scheduling state of the persistent sweep kernel (zeroed by k_trial)
+    long long* S1; long long* S2; int* ovc;   // [Np] per-row fixed-point sums / overlap counts (persistent kernel)
 };
+
+// Order-independent accumulation of a row's partial sums (persistent kernel): the double is split
+// exactly into a multiple of 2^-20 and a remainder below 2^-21 in magnitude, both added as 64-bit
+// integers (the remainder in units of 2^-70: exact for |acc| >= 2^-18, else within 2^-71).  Integer
+// addition is associative, so the total does not depend on which CTA adds first.  Range 2^43.
+__device__ __forceinline__ void accum_row(const Params& p, int i, double acc, int ov) {
+    const long long q1 = __double2ll_rn(__dmul_rn(acc, 0x1.0p20));
+    const double rem = __fma_rn(__ll2double_rn(q1), -0x1.0p-20, acc);
+    const long long q2 = __double2ll_rn(__dmul_rn(rem, 0x1.0p70));
+    atomicAdd((unsigned long long*)(p.S1 + i), (unsigned long long)q1);
+    atomicAdd((unsigned long long*)(p.S2 + i), (unsigned long long)q2);
+    if (ov) atomicAdd(p.ovc + i, ov);
+}
+__device__ __forceinline__ double accum_value(long long s1, long long s2) {
+    return __fma_rn(__ll2double_rn(s2), 0x1.0p-70, __dmul_rn(__ll2double_rn(s1), 0x1.0p-20));
+}
 
 // ------------------------------------------------------------------------------------------
 // a1: trial generation.  Alg. 1 + old position (G1), D = 2 max_disp (G2),
@@ -43,6 +60,7 @@ __global__ void __launch_bounds__(256) k_trial(Params p) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < p.sy_n) p.sy[i] = 0;
     if (i >= p.Np) return;
+    p.S1[i] = 0ll; p.S2[i] = 0ll; p.ovc[i] = 0;
     const double2 xy = p.xy[i];
     const double2 zq = p.zq[i];
     if (i >= p.N) {  // ghost padding: never moves
@@ -274,6 +292,7 @@ __device__ __forceinline__ int blk_index(int t, int s) { return t * (t + 1) / 2 
 
 // one (row tile t, column tile s) unit, executed by one warp; the five arrays are this warp's
 // 32-entry shared-memory staging rows
+template <bool ATOMIC>
 __device__ __forceinline__ void diag_unit(const Params& p, int row0, int nrows, int unit, double2* cxy, double2* czq,
                                           double2* ctxy, double* ch, double* ctz) {
     const int lane = threadIdx.x & 31;
@@ -330,8 +349,12 @@ __device__ __forceinline__ void diag_unit(const Params& p, int row0, int nrows, 
         }
         if (s == t && jj > lane) blk[jj * kTile + lane] = 0.0;
     }
-    p.partD[(size_t)s * p.chunk + r] = bsum;
-    p.ovD[(size_t)s * p.chunk + r] = ovc;
+    if (ATOMIC) {
+        accum_row(p, i, bsum, ovc);
+    } else {
+        p.partD[(size_t)s * p.chunk + r] = bsum;
+        p.ovD[(size_t)s * p.chunk + r] = ovc;
+    }
     if (s <= t) {
         p.OVold[(size_t)r * W + s] = ovo;
         p.OVnew[(size_t)r * W + s] = ovn;
@@ -343,7 +366,7 @@ __global__ void __launch_bounds__(256) k_diag(Params p, int row0, int nrows) {
     __shared__ double2 cxy[8][32], czq[8][32], ctxy[8][32];
     __shared__ double ch[8][32], ctz[8][32];
     const int w = threadIdx.x >> 5;
-    diag_unit(p, row0, nrows, blockIdx.x * 8 + w, cxy[w], czq[w], ctxy[w], ch[w], ctz[w]);
+    diag_unit<false>(p, row0, nrows, blockIdx.x * 8 + w, cxy[w], czq[w], ctxy[w], ch[w], ctz[w]);
 }
 
 // ------------------------------------------------------------------------------------------

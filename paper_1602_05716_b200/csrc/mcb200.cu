@@ -34,7 +34,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t xy, zq, hh, lbq, txy, tz, lnu, wall, partA, ovA, partD, ovD, Dblk, OVold, OVnew, log_dE, log_flags,
-        st, epart, centres, ccount, stage_pos, Efar, ovfar, partF, ovF, sy, total;
+        st, epart, centres, ccount, stage_pos, S1, S2, ovc, sy, dbg, total;
 };
 
 int padded(int64_t N) { return (int)((N + kTile - 1) / kTile * kTile); }
@@ -52,9 +52,9 @@ Layout make_layout(int64_t N) {
     L.partD = take(2 * nt * kChunkMax * 8); L.ovD = take(2 * nt * kChunkMax * 4);
     L.Dblk = take(2 * (nt * (nt + 1) / 2) * kTile * kTile * 8);
     L.OVold = take((size_t)2 * kChunkMax * nt * 4); L.OVnew = take((size_t)2 * kChunkMax * nt * 4);
-    L.Efar = take((size_t)2 * kChunkMax * 8); L.ovfar = take((size_t)2 * kChunkMax * 4);
-    L.partF = take((size_t)2 * kMaxFixSlots * kChunkMax * 8); L.ovF = take((size_t)2 * kMaxFixSlots * kChunkMax * 4);
+    L.S1 = take(Np * 8); L.S2 = take(Np * 8); L.ovc = take(Np * 4);
     L.sy = take((size_t)(kSyHdr + 4 * (Np / 256 + 1)) * 4);
+    L.dbg = take(16 * 8);
     L.log_dE = take(Np * 8); L.log_flags = take(Np);
     L.st = take(sizeof(DevState));
     L.epart = take((size_t)kEnergySlices * Np * 8 + 8);
@@ -80,6 +80,9 @@ struct mc_handle {
     bool overlap = true;
     int engine = 1;          // 1: one persistent kernel per sweep (persist.cuh); 0: kernels per chunk in a graph
     int prows = 4;           // rows per consumer thread of the persistent kernel (chunk = 256 * prows)
+    int pfarcols = 128;      // columns per FAR item of the persistent kernel
+    int pnear = 16;          // worker CTAs of the persistent kernel that serve FIX and DIAG items only
+    bool debug = false;      // collect the cycle counters of mc_debug_counters
     int pgrid = 0;           // CTAs of the persistent kernel (0: not yet configured)
     int bulk_rows = 1;       // rows per consumer thread of k_bulk (1 or 2)
     int bulk_ctas = 2;       // k_bulk CTAs per SM the grid is sized for
@@ -244,11 +247,12 @@ int launch_sweep_kernel(mc_handle* h, cudaStream_t s) {
     a.C = 256 * ROWS;
     a.p.chunk = a.C;
     a.nchunks = (a.p.Np + a.C - 1) / a.C;
-    a.nworkers = std::max(1, h->pgrid - 1);
+    a.nnear = std::min(h->pnear, std::max(0, h->pgrid - 4));
+    a.farcols = h->pfarcols;
     a.sy = h->p.sy;
     char* w = h->ws;
-    a.Efar = (double*)(w + h->L.Efar); a.ovfar = (int*)(w + h->L.ovfar);
-    a.partF = (double*)(w + h->L.partF); a.ovF = (int*)(w + h->L.ovF);
+    a.dbg = h->debug ? (long long*)(w + h->L.dbg) : nullptr;
+    if (a.dbg) CUDA_TRY(cudaMemsetAsync(a.dbg, 0, 16 * 8, s));
     void* args[] = {(void*)&a};
     CUDA_TRY(cudaLaunchCooperativeKernel((void*)kern, dim3(h->pgrid), dim3(kPThreads), args, (size_t)smem, s));
     return MC_OK;
@@ -355,6 +359,7 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     p.log_dE = (double*)(w + L.log_dE); p.log_flags = (unsigned char*)(w + L.log_flags);
     p.st = (DevState*)(w + L.st);
     p.sy = (int*)(w + L.sy);
+    p.S1 = (long long*)(w + L.S1); p.S2 = (long long*)(w + L.S2); p.ovc = (int*)(w + L.ovc);
     p.sy_n = kSyHdr + 4 * (p.Np / 256 + 1);
     h->prows = p.Np >= 16384 ? 4 : (p.Np >= 2048 ? 2 : 1);
     p.R = cavity_R; p.lB = bjerrum_length; p.max_disp = max_disp; p.seed = seed;
@@ -633,6 +638,14 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     } else if (!std::strcmp(key, "engine")) {
         if (value != 0 && value != 1) return fail(MC_EINVAL, "engine must be 0 or 1");
         h->engine = (int)value;
+    } else if (!std::strcmp(key, "far_cols")) {
+        if (value < 8 || value > 65536 || value % 8) return fail(MC_EINVAL, "far_cols must be a multiple of 8 in 8..65536");
+        h->pfarcols = (int)value;
+    } else if (!std::strcmp(key, "pnear")) {
+        if (value < 0 || value > 128) return fail(MC_EINVAL, "pnear must be in 0..128");
+        h->pnear = (int)value;
+    } else if (!std::strcmp(key, "debug")) {
+        h->debug = value != 0;
     } else if (!std::strcmp(key, "prows")) {
         if (value != 1 && value != 2 && value != 4) return fail(MC_EINVAL, "prows must be 1, 2 or 4");
         h->prows = (int)value;
@@ -653,6 +666,13 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
         return fail(MC_EINVAL, std::string("unknown option ") + key);
     }
     drop_graph(h);
+    return MC_OK;
+}
+
+int mc_debug_counters(mc_handle* h, int64_t* out16_host) {
+    if (!h || !out16_host) return fail(MC_EINVAL, "null argument");
+    CUDA_TRY(cudaMemcpyAsync(out16_host, h->ws + h->L.dbg, 16 * 8, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
     return MC_OK;
 }
 

@@ -2,42 +2,42 @@
 //
 // grid = 2 CTAs per SM, all co-resident (cooperative launch).  CTA 0 is the chain: it resolves the
 // sweep's N decisions in ascending order.  Every other CTA is a worker that
-// pulls items from two queues kept in global memory:
-//   normal queue, in chunk order c = 0, 1, ...:
-//     DIAG(c)  speculative corrections inside chunk c (as k_diag)                     (a2/a3)
-//     FAR(c)   rows of chunk c x a slice of the columns outside chunks c-1 and c       (a2)
-//              needs the chain to have finished chunk c-2
-//   urgent queue:
-//     FIX(c)   rows of chunk c x 16 columns of chunk c-1 at their final positions      (a2)
-//              available as soon as the chain has published those columns' row group
-// Partial sums go to fixed slots, so the result does not depend on which CTA ran which item.
-// The chain CTA: warp 0 decides (ballot per step, as k_chain); warps 1..8 each own row tiles
-// t = w-1 (mod 8): they gather the tile's base sum, add the corrections of all column tiles
-// s <= t-2 as their accept masks appear, and hand the tile over through shared memory together
-// with the two blocks D(t,t-1), D(t,t) the chain warp applies itself (one bulk copy).
+// pulls items from three queues (ticket counters in global memory):
+//   DIAG(c)  speculative corrections inside chunk c (as k_diag)                        (a2/a3)
+//   FAR(c)   rows of chunk c x a slice of the columns outside chunks c-1 and c          (a2)
+//            DIAG and FAR of chunk c are released when the chain has finished chunk c-2
+//   FIX(c)   rows of chunk c x 16 columns of chunk c-1 at their final positions         (a2)
+//            urgent: exists as soon as the chain has published those columns' row group
+// Every item adds its rows' partial sums into per-row 64-bit fixed-point accumulators with integer
+// atomics (accum_row): integer addition is associative, so the sums -- and with them every accept
+// bit -- do not depend on which CTA ran which item or in what order.
+// The chain CTA: warp 0 decides (one ballot per step, Alg. 4); warps 1..7 each
+// own row tiles t = w-1 (mod 7): they read the tile's base sum, add the corrections of all column
+// tiles s <= t-2 as their accept masks appear, and hand the tile over through shared memory with
+// the two blocks D(t,t-1), D(t,t) the chain warp applies itself (one bulk copy); warp 8 commits
+// the accepted moves, writes the trial log and publishes progress to the workers.
 #pragma once
 #include "kernels.cuh"
 
 namespace mcb {
 
-constexpr int kPThreads = kBulkThreads + 32;   // 8 consumer warps + 1 producer warp
+constexpr int kPThreads = kBulkThreads + 32;   // workers: 8 consumer warps + 1 producer warp
 constexpr int kGroup = 128;                    // rows per published progress step of the chain
 constexpr int kFixCols = 16;                   // columns per FIX item
 constexpr int kRing = 4;                       // hand-off ring depth of the chain CTA
-constexpr int kHelpers = 8;
-constexpr int kMaxFixSlots = kChunkMax / kFixCols;
+constexpr int kHelpers = 7;
 
 // scheduling state in global memory; zeroed by k_trial at the start of every sweep
-enum { kSyTicket = 0, kSyUTicket = 1, kSyGroups = 2, kSyHdr = 4 };
+enum { kSyTicket = 0, kSyUTicket = 1, kSyGroups = 2, kSyChainSm = 3, kSyDTicket = 4, kSyHdr = 8 };
 
 struct PArgs {
     Params p;
     int C;            // rows per chunk = 256 * ROWS
     int nchunks;
-    int nworkers;     // target number of FAR slices per chunk
-    int* sy;          // [kSyHdr + 4 * nchunks]: header, far_done, far_ready, diag_done, fix_done
-    double* Efar; int* ovfar;   // [2][kChunkMax]     reduced FAR sums of a chunk
-    double* partF; int* ovF;    // [2][kMaxFixSlots][kChunkMax]
+    int farcols;      // target columns per FAR item (multiple of 8)
+    int nnear;        // worker CTAs 1..nnear serve FIX and DIAG only
+    int* sy;          // [kSyHdr + 3 * nchunks]: header, far_done, diag_done, fix_done
+    long long* dbg;   // [16] diagnostic cycle counters (see mc_debug_counters), may be null
 };
 
 __host__ __device__ inline int chunk_rows(int Np, int C, int c) { return min(C, Np - c * C); }
@@ -45,19 +45,10 @@ __host__ __device__ inline int far_cols(int Np, int C, int c) {
     const int row0 = c * C, prev0 = c > 0 ? row0 - C : row0;
     return Np - (row0 + chunk_rows(Np, C, c) - prev0);
 }
-__host__ __device__ inline int far_slices(int ncols, int nworkers) {
-    int n = ncols / 64;                      // at least 64 columns per slice
-    if (n > nworkers) n = nworkers;
-    if (n > kMaxSlices) n = kMaxSlices;
-    if (n < 1 && ncols > 0) n = 1;
-    return n;
-}
+__host__ __device__ inline int far_slices(int ncols, int farcols) { return (ncols + farcols - 1) / farcols; }
 __host__ __device__ inline int diag_items(int nrows) {
     const int nt = nrows / kTile;
     return (nt * nt + 7) / 8;
-}
-__host__ __device__ inline int normal_items(int Np, int C, int nworkers, int c) {
-    return diag_items(chunk_rows(Np, C, c)) + far_slices(far_cols(Np, C, c), nworkers);
 }
 
 __device__ __forceinline__ int ld_acquire(const int* p) {
@@ -69,6 +60,14 @@ __device__ __forceinline__ void st_release(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ double2 ldcg2(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void spin_until_ge(const int* p, int v) {
+    while (ld_acquire(p) < v) __nanosleep(64);
+}
 
 // shared memory of one CTA: workers use the column ring, the chain CTA the hand-off ring
 struct HandOff {
@@ -78,6 +77,8 @@ struct HandOff {
     double tz[kTile];
     unsigned ovoP[kTile], ovnP[kTile], ovoD[kTile], ovnD[kTile];
     unsigned veto[kTile];
+    double out_dE[kTile];          // written by the chain warp, read by the publisher
+    unsigned out_flags[kTile];
 };
 
 struct __align__(128) PShared {
@@ -90,21 +91,35 @@ struct __align__(128) PShared {
         HandOff ho[kRing];
     } u;
     uint64_t full_bar[kStages], empty_bar[kStages];
-    uint64_t ho_bar[kRing];            // tile handed over (helper arrivals + bulk-copy bytes)
+    uint64_t ho_bar[kRing];               // tile handed over (2 helper arrivals + bulk-copy bytes)
+    uint64_t p_bar[kRing];                // publisher done with the slot
     uint64_t a_bar[2][kChunkMax / kTile]; // accept mask of tile t of a chunk (by chunk parity) published
     unsigned sA[2][kChunkMax / kTile];
     int item[4];
 };
 
+__device__ __forceinline__ int* sy_far_done(const PArgs& a) { return a.sy + kSyHdr; }
+__device__ __forceinline__ int* sy_diag_done(const PArgs& a) { return a.sy + kSyHdr + a.nchunks; }
+__device__ __forceinline__ int* sy_fix_done(const PArgs& a) { return a.sy + kSyHdr + 2 * a.nchunks; }
+
+// per-chunk view of the scratch double-buffered by chunk parity
+struct ChunkBufs {
+    double* Dblk;                       // [nt (nt + 1) / 2][32][32]
+    unsigned* OVold; unsigned* OVnew;   // [C][C / 32]
+};
+__device__ __forceinline__ ChunkBufs chunk_bufs(const PArgs& a, int c) {
+    const size_t b = (size_t)(c & 1);
+    const size_t nt = kChunkMax / kTile;
+    ChunkBufs B;
+    B.Dblk = a.p.Dblk + b * (nt * (nt + 1) / 2) * (kTile * kTile);
+    B.OVold = a.p.OVold + b * kChunkMax * nt;
+    B.OVnew = a.p.OVnew + b * kChunkMax * nt;
+    return B;
+}
+
 }  // namespace mcb
 
 namespace mcb {
-
-__device__ __forceinline__ double2 ldcg2(const double2* p) {
-    double2 v;
-    asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
-    return v;
-}
 
 // exact overlap re-check with L2 loads (columns may have been rewritten by the chain during this kernel)
 __device__ __noinline__ int recheck_overlap_cg(const double2* xy, const double2* zq, const double* hh, double2 t,
@@ -122,17 +137,15 @@ __device__ __noinline__ int recheck_overlap_cg(const double2* xy, const double2*
 }
 
 // FAR / FIX item: all rows of the chunk (ROWS per consumer thread) x virtual columns [v0, v1) of
-// [cbeg, cend) minus [gap0, gap1).  Same inner loop as k_bulk; the mbarrier ring persists across
-// items (kring = stages used so far, identical in the producer and in every consumer).
+// the column space that starts at cbeg and skips [gap0, gap1).  Same inner loop as k_bulk; the
+// mbarrier ring persists across items (kring = stages used so far, identical in every thread).
 template <int ROWS, bool UNIFORM>
 __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned& kring, int row0, int nrows,
-                                          int cbeg, int cend, int gap0, int gap1, int v0, int v1, double* part,
-                                          int* ovout) {
+                                          int cbeg, int gap0, int gap1, int v0, int v1) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int kConsumerWarps = kBulkThreads / 32;
     const int gap = gap1 - gap0;
     const int gapv = gap0 - cbeg;
-    (void)cend;
 
     if (warp == kConsumerWarps) {
         if (lane == 0) {
@@ -151,8 +164,7 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
                 v += cnt;
             }
         }
-        // every thread advances the ring counter identically
-        for (int v = v0; v < v1; ++kring) {
+        for (int v = v0; v < v1; ++kring) {   // every thread advances the ring counter identically
             const int lim = (v < gapv) ? min(v1, gapv) : v1;
             v += min(kColTile, lim - v);
         }
@@ -216,10 +228,7 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
         int ov = key < 0 ? 1 : 0;
         if (r < nrows && key >= -kOvBand && key <= kOvBand)
             ov = recheck_overlap_cg(p.xy, p.zq, p.hh, p.txy[row0 + r], p.tz[row0 + r], R[u].h, v0, v1, cbeg, gapv, gap);
-        if (r < nrows) {
-            part[r] = R[u].acc;
-            ovout[r] = ov;
-        }
+        if (r < nrows) accum_row(p, row0 + r, R[u].acc, ov);
     }
 }
 
@@ -227,43 +236,11 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
 
 namespace mcb {
 
-// per-chunk view of the double-buffered scratch (parity b = c & 1)
-struct ChunkBufs {
-    double* partA; int* ovA;       // [slices][C]
-    double* Efar; int* ovfar;      // [C]
-    double* partF; int* ovF;       // [C / kFixCols][C]
-    double* partD; int* ovD;       // [C / 32][C]
-    double* Dblk;                  // [nt (nt + 1) / 2][32][32]
-    unsigned* OVold; unsigned* OVnew;   // [C][C / 32]
-};
-
-__device__ __forceinline__ ChunkBufs chunk_bufs(const PArgs& a, int c) {
-    const size_t b = (size_t)(c & 1);
-    const size_t nt = kChunkMax / kTile;
-    ChunkBufs B;
-    B.partA = a.p.partA + b * kMaxSlices * kChunkMax;  B.ovA = a.p.ovA + b * kMaxSlices * kChunkMax;
-    B.Efar = a.Efar + b * kChunkMax;                   B.ovfar = a.ovfar + b * kChunkMax;
-    B.partF = a.partF + b * kMaxFixSlots * kChunkMax;  B.ovF = a.ovF + b * kMaxFixSlots * kChunkMax;
-    B.partD = a.p.partD + b * nt * kChunkMax;          B.ovD = a.p.ovD + b * nt * kChunkMax;
-    B.Dblk = a.p.Dblk + b * (nt * (nt + 1) / 2) * (kTile * kTile);
-    B.OVold = a.p.OVold + b * kChunkMax * nt;          B.OVnew = a.p.OVnew + b * kChunkMax * nt;
-    return B;
-}
-
-__device__ __forceinline__ int* sy_far_done(const PArgs& a) { return a.sy + kSyHdr; }
-__device__ __forceinline__ int* sy_far_ready(const PArgs& a) { return a.sy + kSyHdr + a.nchunks; }
-__device__ __forceinline__ int* sy_diag_done(const PArgs& a) { return a.sy + kSyHdr + 2 * a.nchunks; }
-__device__ __forceinline__ int* sy_fix_done(const PArgs& a) { return a.sy + kSyHdr + 3 * a.nchunks; }
-
-__device__ __forceinline__ void spin_until_ge(const int* p, int v) {
-    while (ld_acquire(p) < v) __nanosleep(64);
-}
-
 // ------------------------------------------------------------------------------------------
 // helper warp of the chain CTA: prepares row tile t of chunk c and hands it over
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, const ChunkBufs& B, int c, int t,
-                                                  int row0, int nt, int nf, int nfix, int gt) {
+                                                  int row0, int gt) {
     const int lane = threadIdx.x & 31;
     const int C = a.C, W = C / kTile;
     const int r = t * kTile + lane, i = row0 + r;
@@ -271,25 +248,9 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
     HandOff& ho = sh.u.ho[slot];
     const unsigned apar = (unsigned)(c >> 1) & 1u;
 
-    // base sum: FAR (reduced) + FIX slots + DIAG slots, fixed order
-    double e4[4] = {0.0, 0.0, 0.0, 0.0};
-    int ovc = 0;
-    if (nf > 0) { e4[0] = __ldcg(B.Efar + r); ovc = __ldcg(B.ovfar + r); }
-    for (int j = 0; j < nfix; j += 4) {
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            e4[u] = __dadd_rn(e4[u], __ldcg(B.partF + (size_t)(j + u) * C + r));
-            ovc += __ldcg(B.ovF + (size_t)(j + u) * C + r);
-        }
-    }
-    for (int s = 0; s < nt; ++s) {
-        e4[s & 3] = __dadd_rn(e4[s & 3], __ldcg(B.partD + (size_t)s * C + r));
-        ovc += __ldcg(B.ovD + (size_t)s * C + r);
-    }
-    double E = __dadd_rn(__dadd_rn(e4[0], e4[1]), __dadd_rn(e4[2], e4[3]));
-    unsigned veto = (unsigned)a.p.wall[i] | (ovc > 0 ? kFlagOverlap : 0u);
-
-    // per-row scalars and the overlap words of the two blocks the chain warp applies itself
+    // base sum of all FAR, FIX and DIAG items of this row
+    double E = accum_value(__ldcg(a.p.S1 + i), __ldcg(a.p.S2 + i));
+    unsigned veto = (unsigned)a.p.wall[i] | (__ldcg(a.p.ovc + i) > 0 ? kFlagOverlap : 0u);
     const double lbq = a.p.lbq[i], lnu = a.p.lnu[i];
     const double2 txy = a.p.txy[i];
     const double tz = a.p.tz[i];
@@ -299,11 +260,8 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
 
     bool staged = false;
     auto stage_blocks = [&]() {
-        // the slot is free once the chain has finished tile gt - kRing
-        if (gt >= kRing) {
-            if (t >= kRing) mbar_wait(&sh.a_bar[c & 1][t - kRing], apar);
-            else mbar_wait(&sh.a_bar[(c - 1) & 1][C / kTile + t - kRing], (unsigned)((c - 1) >> 1) & 1u);
-        }
+        // the slot is free once the publisher is done with tile gt - kRing
+        if (gt >= kRing) mbar_wait(&sh.p_bar[slot], (unsigned)(gt / kRing - 1) & 1u);
         if (lane == 0) {
             const double* src = B.Dblk + (size_t)blk_index(t, t > 0 ? t - 1 : 0) * (kTile * kTile);
             const uint32_t bytes = (t > 0 ? 2u : 1u) * kTile * kTile * 8u;
@@ -316,7 +274,7 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
 
     // corrections of the column tiles s <= t - 2, as their accept masks appear
     for (int s = 0; s + 2 <= t; ++s) {
-        if (!staged && s + kRing >= t) stage_blocks();   // a_bar[t - kRing] is awaited here at the latest
+        if (!staged && s + kRing >= t) stage_blocks();
         mbar_wait(&sh.a_bar[c & 1][s], apar);
         const unsigned A = sh.sA[c & 1][s];
         const double* blk = B.Dblk + (size_t)blk_index(t, s) * (kTile * kTile);
@@ -340,6 +298,70 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
     if (lane == 0) mbar_arrive(&sh.ho_bar[slot]);
 }
 
+// ------------------------------------------------------------------------------------------
+// publisher warp of the chain CTA (a4): commit x <- x~ for the accepted trials, trial log, counters,
+// and the progress counter the workers' FIX and release conditions read
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void chain_publisher(const PArgs& a, PShared& sh) {
+    const int lane = threadIdx.x & 31;
+    const Params& p = a.p;
+    const int C = a.C, GPC = C / kGroup, ntfull = C / kTile;
+    unsigned long long n_acc = 0, n_ov = 0, n_wall = 0, n_tie = 0;
+    double e_lane = 0.0;
+    for (int c = 0; c < a.nchunks; ++c) {
+        const int row0 = c * C, nt = chunk_rows(p.Np, C, c) / kTile;
+        for (int t = 0; t < nt; ++t) {
+            const int gt = c * ntfull + t, slot = gt % kRing;
+            mbar_wait(&sh.a_bar[c & 1][t], (unsigned)(c >> 1) & 1u);
+            const HandOff& ho = sh.u.ho[slot];
+            const int i = row0 + t * kTile + lane;
+            const unsigned fl = ho.out_flags[lane];
+            const double dE = ho.out_dE[lane];
+            if (fl & kFlagAccept) {
+                p.xy[i] = ho.txy[lane];
+                p.zq[i].x = ho.tz[lane];
+                e_lane = __dadd_rn(e_lane, dE);
+            }
+            p.log_dE[i] = dE;
+            p.log_flags[i] = (unsigned char)fl;
+            if (i < p.N) {
+                n_acc += (fl & kFlagAccept) ? 1 : 0;
+                n_ov += (fl & kFlagOverlap) ? 1 : 0;
+                n_wall += (fl & kFlagWall) ? 1 : 0;
+                n_tie += (fl & kFlagNearTie) ? 1 : 0;
+            }
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&sh.p_bar[slot]);
+                const int rows_done = (t + 1) * kTile;
+                if (rows_done % kGroup == 0 || t + 1 == nt) {
+                    __threadfence();
+                    fence_proxy_async();
+                    st_release(a.sy + kSyGroups, c * GPC + (rows_done + kGroup - 1) / kGroup);
+                }
+            }
+        }
+    }
+    // fixed-order reductions over the lanes
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        n_acc += __shfl_xor_sync(0xffffffffu, n_acc, o);
+        n_ov += __shfl_xor_sync(0xffffffffu, n_ov, o);
+        n_wall += __shfl_xor_sync(0xffffffffu, n_wall, o);
+        n_tie += __shfl_xor_sync(0xffffffffu, n_tie, o);
+    }
+    const double e_run = warp_sum(e_lane);
+    if (lane == 0) {
+        DevState* st = p.st;
+        st->accepted += n_acc;
+        st->veto_overlap += n_ov;
+        st->veto_wall += n_wall;
+        st->near_ties += n_tie;
+        st->E_run += e_run;
+        st->sweep += 1ull;
+    }
+}
+
 }  // namespace mcb
 
 namespace mcb {
@@ -351,40 +373,46 @@ namespace mcb {
 __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const Params& p = a.p;
-    const int C = a.C, GPC = C / kGroup;
+    const int C = a.C;
     const int ntfull = C / kTile;
 
+    if (warp == kHelpers + 1) {
+        chain_publisher(a, sh);
+        return;
+    }
     if (warp >= 1) {
         // ---------------- helpers ----------------
         const int h = warp - 1;
         for (int c = 0; c < a.nchunks; ++c) {
             const int row0 = c * C, nrows = chunk_rows(p.Np, C, c), nt = nrows / kTile;
-            const int nf = far_slices(far_cols(p.Np, C, c), a.nworkers);
-            const int nfix = c > 0 ? C / kFixCols : 0;
             if (h >= nt) continue;
             if (lane == 0) {
-                if (nf > 0) spin_until_ge(sy_far_ready(a) + c, 1);
+                const long long t0 = clock64();
+                spin_until_ge(sy_far_done(a) + c, far_slices(far_cols(p.Np, C, c), a.farcols));
                 spin_until_ge(sy_diag_done(a) + c, diag_items(nrows));
-                if (nfix > 0) spin_until_ge(sy_fix_done(a) + c, nfix);
+                const long long t1 = clock64();
+                if (c > 0) spin_until_ge(sy_fix_done(a) + c, C / kFixCols);
+                if (h == 0 && a.dbg) { a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t1; }
             }
             __syncwarp();
             const ChunkBufs B = chunk_bufs(a, c);
-            for (int t = h; t < nt; t += kHelpers) chain_helper_tile(a, sh, B, c, t, row0, nt, nf, nfix, c * ntfull + t);
+            for (int t = h; t < nt; t += kHelpers) chain_helper_tile(a, sh, B, c, t, row0, c * ntfull + t);
         }
         return;
     }
 
     // ---------------- the chain warp ----------------
-    unsigned long long n_acc = 0, n_ov = 0, n_wall = 0, n_tie = 0;
-    double e_run = 0.0;
+    long long w_first = 0, w_other = 0;
+    const long long t_start = clock64();
     for (int c = 0; c < a.nchunks; ++c) {
-        const int row0 = c * C, nrows = chunk_rows(p.Np, C, c), nt = nrows / kTile;
+        const int nt = chunk_rows(p.Np, C, c) / kTile;
         unsigned Ap = 0u;
         for (int t = 0; t < nt; ++t) {
             const int gt = c * ntfull + t, slot = gt % kRing;
+            const long long tw = clock64();
             mbar_wait(&sh.ho_bar[slot], (unsigned)(gt / kRing) & 1u);
-            const HandOff& ho = sh.u.ho[slot];
-            const int i = row0 + t * kTile + lane;
+            if (t == 0) w_first += clock64() - tw; else w_other += clock64() - tw;
+            HandOff& ho = sh.u.ho[slot];
             const double lbq = ho.lbq[lane], lnu = ho.lnu[lane];
             double Eu = ho.E[lane];
             const unsigned vflags = ho.veto[lane];
@@ -401,12 +429,14 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
             double Es = __fma_rn(lbq, Eu, lnu);
             const unsigned ovo = ho.ovoD[lane], ovn = ho.ovnD[lane];
             const double* diag = ho.D + kTile * kTile;
+            bool veto = wallv || ovv;
             unsigned A = 0u;
 #pragma unroll
             for (int j = 0; j < kTile; ++j) {
                 const double dj = diag[j * kTile + lane];   // 0 for lanes <= j
                 const double djs = __dmul_rn(lbq, dj);
-                const bool ok = !wallv && !ovv && (Es < 0.0);
+                // Es < 0 read off the sign bit (Es is never -0: ln u < 0 strictly, and x + y = -0 needs x = y = -0)
+                const bool ok = !veto && (__double2hiint(Es) < 0);
                 const unsigned bal = __ballot_sync(0xffffffffu, ok);
                 const bool bit = ((bal >> j) & 1u) != 0u;
                 A |= (bit ? 1u : 0u) << j;
@@ -414,47 +444,25 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
                     Es = __dadd_rn(Es, djs);
                     Eu = __dadd_rn(Eu, dj);
                 }
-                ovv = ovv || ((((bit ? ovn : ovo) >> j) & 1u) != 0u);  // bits >= lane are 0
+                const bool hit = (((bit ? ovn : ovo) >> j) & 1u) != 0u;  // bits >= lane are 0
+                veto = veto || hit;
+                ovv = ovv || hit;
             }
             const bool acc = ((A >> lane) & 1u) != 0u;
-            const double dE = __dmul_rn(lbq, Eu);
-            const bool tie = !wallv && !ovv && (fabs(Es) < 1e-8);
-            if (acc) {   // commit: x <- x~ (a4)
-                p.xy[i] = ho.txy[lane];
-                p.zq[i].x = ho.tz[lane];
-            }
-            p.log_dE[i] = dE;
-            p.log_flags[i] = (unsigned char)((acc ? kFlagAccept : 0u) | (ovv ? kFlagOverlap : 0u) |
-                                             (wallv ? kFlagWall : 0u) | (tie ? kFlagNearTie : 0u));
-            const bool real = i < p.N;
-            n_acc += __popc(A);
-            n_ov += __popc(__ballot_sync(0xffffffffu, real && ovv));
-            n_wall += __popc(__ballot_sync(0xffffffffu, real && wallv));
-            n_tie += __popc(__ballot_sync(0xffffffffu, real && tie));
-            e_run += warp_sum(acc ? dE : 0.0);
+            const bool tie = !veto && (fabs(Es) < 1e-8);
+            ho.out_dE[lane] = __dmul_rn(lbq, Eu);
+            ho.out_flags[lane] = (acc ? kFlagAccept : 0u) | (ovv ? kFlagOverlap : 0u) | (wallv ? kFlagWall : 0u) |
+                                 (tie ? kFlagNearTie : 0u);
             Ap = A;
             if (lane == 0) sh.sA[c & 1][t] = A;
             __syncwarp();
-            if (lane == 0) {
-                mbar_arrive(&sh.a_bar[c & 1][t]);
-                // publish the committed rows to the workers, one group (or the chunk's end) at a time
-                const int rows_done = (t + 1) * kTile;
-                if (rows_done % kGroup == 0 || t + 1 == nt) {
-                    __threadfence();
-                    fence_proxy_async();
-                    st_release(a.sy + kSyGroups, c * GPC + (rows_done + kGroup - 1) / kGroup);
-                }
-            }
+            if (lane == 0) mbar_arrive(&sh.a_bar[c & 1][t]);
         }
     }
-    if (lane == 0) {
-        DevState* st = p.st;
-        st->accepted += n_acc;
-        st->veto_overlap += n_ov;
-        st->veto_wall += n_wall;
-        st->near_ties += n_tie;
-        st->E_run += e_run;
-        st->sweep += 1ull;
+    if (lane == 0 && a.dbg) {
+        a.dbg[0] = clock64() - t_start;   // chain warp: whole sweep
+        a.dbg[1] = w_first;               //   waiting for the first tile of a chunk
+        a.dbg[2] = w_other;               //   waiting for the other tiles (helpers late)
     }
 }
 
@@ -464,19 +472,52 @@ namespace mcb {
 
 enum { kItemExit = 0, kItemDiag = 1, kItemFar = 2, kItemFix = 3 };
 
-// Thread 0 of a worker CTA: claim the next item.  Urgent items first; a claimed normal ticket whose
-// chunk is not yet released by the chain is kept while urgent items are served (the chain can only
-// be waiting for items that are already claimed or urgent, so nobody starves).
+// Thread 0 of a worker CTA claims the next item.  Three queues, each a ticket counter in global
+// memory: FIX (urgent; an item exists once the chain has published its columns), DIAG and FAR (in
+// chunk order; chunk c is released when the chain has finished chunk c-2).  "Near" workers (the
+// first a.nnear worker CTAs) serve FIX and DIAG only, so that the chain never waits for a CTA that
+// is busy with a long FAR item; the others serve FAR and help with FIX/DIAG whenever their FAR
+// ticket is not released yet.  A claimed ticket is kept until it is released, and a held DIAG
+// ticket goes before FAR: every item the chain can be waiting for is then either claimed by a
+// CTA that will run it next, or still claimable.
 struct Cursor {
-    int ticket;     // claimed normal ticket, -1 if none
-    int c, base;    // chunk the ticket cursor is in, first ticket of that chunk
+    int ticket;     // claimed ticket, -1 if none
+    int c, base;    // chunk the cursor is in, first ticket of that chunk
 };
 
-__device__ __forceinline__ void fetch_item(const PArgs& a, Cursor& cur, int* item) {
+template <bool FAR>
+__device__ __forceinline__ int items_of(const PArgs& a, int c) {
+    return FAR ? far_slices(far_cols(a.p.Np, a.C, c), a.farcols) : diag_items(chunk_rows(a.p.Np, a.C, c));
+}
+
+// true if an item of this queue was taken (written to item[]); done = queue exhausted
+template <bool FAR>
+__device__ __forceinline__ bool try_queue(const PArgs& a, Cursor& cur, int* item, bool& done) {
+    if (cur.ticket < 0 && cur.c < a.nchunks) {
+        cur.ticket = atomicAdd(a.sy + (FAR ? kSyTicket : kSyDTicket), 1);
+        while (cur.c < a.nchunks && cur.ticket >= cur.base + items_of<FAR>(a, cur.c)) {
+            cur.base += items_of<FAR>(a, cur.c);
+            ++cur.c;
+        }
+    }
+    done = cur.c >= a.nchunks;
+    if (done) return false;
+    if (cur.c >= 2 && ld_acquire(a.sy + kSyGroups) < (cur.c - 1) * (a.C / kGroup)) return false;
+    item[0] = FAR ? kItemFar : kItemDiag;
+    item[1] = cur.c;
+    item[2] = cur.ticket - cur.base;
+    cur.ticket = -1;
+    return true;
+}
+
+__device__ __forceinline__ void fetch_item(const PArgs& a, Cursor& cfar, Cursor& cdiag, bool near, int* item) {
     const int C = a.C, GPC = C / kGroup, fix_per_chunk = C / kFixCols;
     const int total_urgent = (a.nchunks - 1) * fix_per_chunk;
     int* sy = a.sy;
     for (;;) {
+        bool far_done = true, diag_done = false;
+        if (cdiag.ticket >= 0 && try_queue<false>(a, cdiag, item, diag_done)) return;
+        if (!near && try_queue<true>(a, cfar, item, far_done)) return;
         const int u = *(volatile int*)(sy + kSyUTicket);
         if (u < total_urgent) {
             const int c = 1 + u / fix_per_chunk, j = u % fix_per_chunk;
@@ -489,25 +530,9 @@ __device__ __forceinline__ void fetch_item(const PArgs& a, Cursor& cur, int* ite
                 continue;
             }
         }
-        if (cur.ticket < 0) {
-            cur.ticket = atomicAdd(sy + kSyTicket, 1);
-            while (cur.c < a.nchunks && cur.ticket >= cur.base + normal_items(a.p.Np, C, a.nworkers, cur.c)) {
-                cur.base += normal_items(a.p.Np, C, a.nworkers, cur.c);
-                ++cur.c;
-            }
-        }
-        if (cur.c >= a.nchunks) {           // normal queue exhausted
-            if (u >= total_urgent) { item[0] = kItemExit; return; }
-        } else if (cur.c < 2 || ld_acquire(sy + kSyGroups) >= (cur.c - 1) * GPC) {
-            const int k = cur.ticket - cur.base;
-            const int nd = diag_items(chunk_rows(a.p.Np, C, cur.c));
-            item[0] = k < nd ? kItemDiag : kItemFar;
-            item[1] = cur.c;
-            item[2] = k < nd ? k : k - nd;
-            cur.ticket = -1;
-            return;
-        }
-        __nanosleep(200);
+        if (try_queue<false>(a, cdiag, item, diag_done)) return;
+        if (far_done && diag_done && u >= total_urgent) { item[0] = kItemExit; return; }
+        __nanosleep(100);
     }
 }
 
@@ -524,86 +549,72 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
             mbar_init(&sh.full_bar[s], 1);
             mbar_init(&sh.empty_bar[s], kBulkThreads / 32);
         }
-        for (int s = 0; s < kRing; ++s) mbar_init(&sh.ho_bar[s], 2);
+        for (int s = 0; s < kRing; ++s) { mbar_init(&sh.ho_bar[s], 2); mbar_init(&sh.p_bar[s], 1); }
         for (int s = 0; s < 2 * (kChunkMax / kTile); ++s) mbar_init(&sh.a_bar[0][0] + s, 1);
         mbar_fence_init();
+        // the chain CTA gets its SM to itself: it publishes the SM it runs on, and the worker CTA
+        // that shares that SM retires at once
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        if (blockIdx.x == 0) {
+            st_release(a.sy + kSyChainSm, (int)smid + 1);
+        } else {
+            int v;
+            while ((v = ld_acquire(a.sy + kSyChainSm)) == 0) __nanosleep(100);
+            sh.item[0] = (v == (int)smid + 1) ? 1 : 0;
+        }
     }
     __syncthreads();
-
     if (blockIdx.x == 0) {
         chain_cta(a, sh);
         return;
     }
+    if (sh.item[0] == 1) return;
 
-    Cursor cur{-1, 0, 0};
+    Cursor cfar{-1, 0, 0}, cdiag{-1, 0, 0};
+    const bool near = (int)blockIdx.x <= a.nnear;
     unsigned kring = 0;
     for (;;) {
         __syncthreads();
-        if (tid == 0) fetch_item(a, cur, sh.item);
+        if (tid == 0) {
+            const long long t0 = clock64();
+            fetch_item(a, cfar, cdiag, near, sh.item);
+            if (a.dbg) {
+                atomicAdd((unsigned long long*)a.dbg + 5, (unsigned long long)(clock64() - t0));
+                atomicAdd((unsigned long long*)a.dbg + 6 + sh.item[0], 1ull);   // [6] exits, [7] diag, [8] far, [9] fix
+            }
+        }
         __syncthreads();
         const int type = sh.item[0], c = sh.item[1], k = sh.item[2];
         if (type == kItemExit) break;
         const int row0 = c * C, nrows = chunk_rows(p.Np, C, c);
-        const ChunkBufs B = chunk_bufs(a, c);
         int* counter;
         if (type == kItemDiag) {
             if (warp < 8) {
+                const ChunkBufs B = chunk_bufs(a, c);
                 Params pc = p;
                 pc.chunk = C;
-                pc.partD = B.partD; pc.ovD = B.ovD; pc.Dblk = B.Dblk; pc.OVold = B.OVold; pc.OVnew = B.OVnew;
-                diag_unit(pc, row0, nrows, k * 8 + warp, sh.u.w.cxy[warp], sh.u.w.czq[warp], sh.u.w.ctxy[warp],
-                          sh.u.w.ch[warp], sh.u.w.ctz[warp]);
+                pc.Dblk = B.Dblk; pc.OVold = B.OVold; pc.OVnew = B.OVnew;
+                diag_unit<true>(pc, row0, nrows, k * 8 + warp, sh.u.w.cxy[warp], sh.u.w.czq[warp], sh.u.w.ctxy[warp],
+                                sh.u.w.ch[warp], sh.u.w.ctz[warp]);
             }
             counter = sy_diag_done(a) + c;
         } else if (type == kItemFar) {
             const int prev0 = c > 0 ? row0 - C : row0;
             const int ncols = far_cols(p.Np, C, c);
-            const int nf = far_slices(ncols, a.nworkers);
+            const int nf = far_slices(ncols, a.farcols);
             const int v0 = slice_bound(ncols, nf, k), v1 = slice_bound(ncols, nf, k + 1);
-            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, 0, p.Np, prev0, row0 + nrows, v0, v1,
-                                     B.partA + (size_t)k * C, B.ovA + (size_t)k * C);
+            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, 0, prev0, row0 + nrows, v0, v1);
             counter = sy_far_done(a) + c;
         } else {
             const int cb = row0 - C + k * kFixCols;
-            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, cb + kFixCols, cb, cb, 0, kFixCols,
-                                     B.partF + (size_t)k * C, B.ovF + (size_t)k * C);
+            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, cb, cb, 0, kFixCols);
             counter = sy_fix_done(a) + c;
         }
         __syncthreads();
         if (tid == 0) {
             __threadfence();
-            const int old = atomicAdd(counter, 1);
-            __threadfence();
-            sh.item[3] = old;
-        }
-        if (type != kItemFar) continue;
-        __syncthreads();
-        const int nf = far_slices(far_cols(p.Np, C, c), a.nworkers);
-        if (sh.item[3] != nf - 1) continue;
-        // last FAR item of the chunk: reduce the slots in a fixed order
-        for (int r = tid; r < nrows; r += kPThreads) {
-            double e[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-            int ov = 0;
-            for (int sl = 0; sl < nf; sl += 8) {
-                double v[8];
-                int o[8];
-#pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    const bool in = sl + u < nf;
-                    v[u] = in ? __ldcg(B.partA + (size_t)(sl + u) * C + r) : 0.0;
-                    o[u] = in ? __ldcg(B.ovA + (size_t)(sl + u) * C + r) : 0;
-                }
-#pragma unroll
-                for (int u = 0; u < 8; ++u) { e[u] = __dadd_rn(e[u], v[u]); ov += o[u]; }
-            }
-            B.Efar[r] = __dadd_rn(__dadd_rn(__dadd_rn(e[0], e[1]), __dadd_rn(e[2], e[3])),
-                                  __dadd_rn(__dadd_rn(e[4], e[5]), __dadd_rn(e[6], e[7])));
-            B.ovfar[r] = ov;
-        }
-        __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            st_release(sy_far_ready(a) + c, 1);
+            atomicAdd(counter, 1);
         }
     }
 }
