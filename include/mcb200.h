@@ -40,6 +40,7 @@ extern "C" {
 #define MC_EOUTSIDE (-3) /* an ion sticks out of the cavity in the initial configuration           */
 #define MC_ENOSPACE (-4) /* workspace too small                                                    */
 #define MC_ECUDA (-5)    /* a CUDA runtime call failed, or no sm_100 device                        */
+#define MC_ESTALL (-6)   /* the sweep kernel's watchdog fired (a wait exceeded 2 s): state invalid  */
 
 typedef struct mc_handle mc_handle;
 
@@ -134,6 +135,11 @@ int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_
  * FIX; [5] summed cycles worker CTAs spent fetching items; [6..9] number of exit/DIAG/FAR/FIX
  * items fetched.  Synchronises. */
 int mc_debug_counters(mc_handle* h, int64_t* out16_host);
+
+/* Diagnostics: copies the first n ints of the persistent kernel's scheduling state (ticket
+ * counters, progress counter, per-chunk completion counters) to the host on a stream of its own,
+ * without waiting for the handle's stream (usable while a sweep is running). */
+int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
 
 /* Tuning knobs (diagnostic; defaults are right for B200): key "chunk" = rows resolved per
  * chain kernel (multiple of 32, 32..1024), "graph" = 0/1 use CUDA graphs, "overlap" = 0/1 run

@@ -15,14 +15,14 @@ import torch
 _PKG = Path(__file__).resolve().parent
 _LIBPATH = _PKG / "libmcb200.so"
 
-MC_OK, MC_EINVAL, MC_EOVERLAP, MC_EOUTSIDE, MC_ENOSPACE, MC_ECUDA = 0, -1, -2, -3, -4, -5
-_CODES = {-1: "MC_EINVAL", -2: "MC_EOVERLAP", -3: "MC_EOUTSIDE", -4: "MC_ENOSPACE", -5: "MC_ECUDA"}
+MC_OK, MC_EINVAL, MC_EOVERLAP, MC_EOUTSIDE, MC_ENOSPACE, MC_ECUDA, MC_ESTALL = 0, -1, -2, -3, -4, -5, -6
+_CODES = {-1: "MC_EINVAL", -2: "MC_EOVERLAP", -3: "MC_EOUTSIDE", -4: "MC_ENOSPACE", -5: "MC_ECUDA", -6: "MC_ESTALL"}
 
 EXPORTS = (
     "mc_workspace_bytes", "mc_init", "mc_sweep", "mc_energy", "mc_energy_dev", "mc_pair_hist", "mc_sweep_host",
     "mc_sweep_timed",
     "mc_get_positions", "mc_set_positions", "mc_get_sweep_index", "mc_set_sweep_index", "mc_get_stats",
-    "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option", "mc_debug_counters",
+    "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option", "mc_debug_counters", "mc_debug_peek",
     "mc_get_launch_count",
 )
 
@@ -71,6 +71,7 @@ def load_library() -> C.CDLL:
     lib.mc_set_option.argtypes = [vp, C.c_char_p, i64]
     lib.mc_get_launch_count.argtypes = [vp, C.POINTER(u64)]
     lib.mc_debug_counters.argtypes = [vp, C.POINTER(C.c_int64)]
+    lib.mc_debug_peek.argtypes = [vp, C.POINTER(C.c_int32), C.c_int]
     for name in EXPORTS:
         if name not in ("mc_workspace_bytes", "mc_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -249,6 +250,11 @@ class MCSystem:
     def mc_debug_counters(self) -> list:
         out = (C.c_int64 * 16)()
         _check(self._lib.mc_debug_counters(self._h, out))
+        return list(out)
+
+    def mc_debug_peek(self, n: int) -> list:
+        out = (C.c_int32 * abs(n))()
+        _check(self._lib.mc_debug_peek(self._h, out, n))
         return list(out)
 
     def mc_get_launch_count(self) -> int:

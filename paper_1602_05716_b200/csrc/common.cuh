@@ -24,6 +24,7 @@ struct DevState {
     double E_run;
     int err;        // validation result (0 ok, MC_E* otherwise)
     int d_differs;  // set by k_check_particles if not all diameters are equal
+    int stall;      // set by the persistent sweep kernel's watchdog (a wait exceeded its time limit)
 };
 
 // ---------------------------------------------------------------------------------------------

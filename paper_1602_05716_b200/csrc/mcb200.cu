@@ -53,8 +53,10 @@ Layout make_layout(int64_t N) {
     L.Dblk = take(2 * (nt * (nt + 1) / 2) * kTile * kTile * 8);
     L.OVold = take((size_t)2 * kChunkMax * nt * 4); L.OVnew = take((size_t)2 * kChunkMax * nt * 4);
     L.S1 = take(Np * 8); L.S2 = take(Np * 8); L.ovc = take(Np * 4);
+    take(65536);
     L.sy = take((size_t)(kSyHdr + 4 * (Np / 256 + 1)) * 4);
-    L.dbg = take(16 * 8);
+    take(65536);
+    L.dbg = take(16 * 8 + 2048 * 4);
     L.log_dE = take(Np * 8); L.log_flags = take(Np);
     L.st = take(sizeof(DevState));
     L.epart = take((size_t)kEnergySlices * Np * 8 + 8);
@@ -567,6 +569,7 @@ int mc_get_stats(mc_handle* h, mc_stats* stats_host) {
     stats_host->accepted = st.accepted; stats_host->veto_overlap = st.veto_overlap;
     stats_host->veto_wall = st.veto_wall; stats_host->near_ties = st.near_ties;
     stats_host->E_running = st.E_run;
+    if (st.stall) return fail(MC_ESTALL, "the sweep kernel's watchdog fired: a wait exceeded its time limit");
     return MC_OK;
 }
 
@@ -673,6 +676,18 @@ int mc_debug_counters(mc_handle* h, int64_t* out16_host) {
     if (!h || !out16_host) return fail(MC_EINVAL, "null argument");
     CUDA_TRY(cudaMemcpyAsync(out16_host, h->ws + h->L.dbg, 16 * 8, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return MC_OK;
+}
+
+int mc_debug_peek(mc_handle* h, int32_t* out_host, int n) {
+    if (!h || !out_host || n > h->p.sy_n) return fail(MC_EINVAL, "bad argument");
+    cudaStream_t s2;
+    CUDA_TRY(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
+    if (n < 0) CUDA_TRY(cudaMemcpyAsync(out_host, h->ws + h->L.dbg, (size_t)(-n) * 4, cudaMemcpyDeviceToHost, s2));
+    else
+    CUDA_TRY(cudaMemcpyAsync(out_host, h->p.sy, (size_t)n * 4, cudaMemcpyDeviceToHost, s2));
+    CUDA_TRY(cudaStreamSynchronize(s2));
+    cudaStreamDestroy(s2);
     return MC_OK;
 }
 

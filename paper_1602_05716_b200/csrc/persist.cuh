@@ -11,24 +11,24 @@
 // Every item adds its rows' partial sums into per-row 64-bit fixed-point accumulators with integer
 // atomics (accum_row): integer addition is associative, so the sums -- and with them every accept
 // bit -- do not depend on which CTA ran which item or in what order.
-// The chain CTA: warp 0 decides (one ballot per step, Alg. 4); warps 1..7 each
-// own row tiles t = w-1 (mod 7): they read the tile's base sum, add the corrections of all column
+// The chain CTA: warp 0 decides (one ballot per step, Alg. 4); warps 1..6 each
+// own row tiles t = w-1 (mod 6): they read the tile's base sum, add the corrections of all column
 // tiles s <= t-2 as their accept masks appear, and hand the tile over through shared memory with
-// the two blocks D(t,t-1), D(t,t) the chain warp applies itself (one bulk copy); warp 8 commits
+// the two blocks D(t,t-1), D(t,t) the chain warp applies itself (one bulk copy); warp 7 commits
 // the accepted moves, writes the trial log and publishes progress to the workers.
 #pragma once
 #include "kernels.cuh"
 
 namespace mcb {
 
-constexpr int kPThreads = kBulkThreads + 32;   // workers: 8 consumer warps + 1 producer warp
+constexpr int kPThreads = kBulkThreads;        // workers: 8 consumer warps; thread 0 also feeds the column ring
 constexpr int kGroup = 128;                    // rows per published progress step of the chain
 constexpr int kFixCols = 16;                   // columns per FIX item
 constexpr int kRing = 4;                       // hand-off ring depth of the chain CTA
-constexpr int kHelpers = 7;
+constexpr int kHelpers = 6;
 
 // scheduling state in global memory; zeroed by k_trial at the start of every sweep
-enum { kSyTicket = 0, kSyUTicket = 1, kSyGroups = 2, kSyChainSm = 3, kSyDTicket = 4, kSyHdr = 8 };
+enum { kSyTicket = 0, kSyUTicket = 1, kSyGroups = 2, kSyChainSm = 3, kSyDTicket = 4, kSyAbort = 5, kSyHdr = 8 };
 
 struct PArgs {
     Params p;
@@ -65,8 +65,41 @@ __device__ __forceinline__ double2 ldcg2(const double2* p) {
     asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
     return v;
 }
-__device__ __forceinline__ void spin_until_ge(const int* p, int v) {
-    while (ld_acquire(p) < v) __nanosleep(64);
+// Watchdog: no wait in this kernel may last longer than kWaitLimitNs.  A thread whose wait does
+// raises the abort flag (and DevState::stall, which the host reports as MC_ESTALL) and exits;
+// every other waiting thread sees the flag and exits too, so a scheduling bug can never hang the GPU.
+constexpr unsigned long long kWaitLimitNs = 2000000000ull;
+struct Watch {
+    int* sy;
+    DevState* st;
+};
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __noinline__ void wd_check(const Watch& w, unsigned long long t0) {
+    if (*(volatile int*)(w.sy + kSyAbort) == 0) {
+        if (global_ns() - t0 < kWaitLimitNs) return;
+        *(volatile int*)(w.sy + kSyAbort) = 1;
+        *(volatile int*)(&w.st->stall) = 1;
+        __threadfence();
+    }
+    asm volatile("exit;");
+}
+__device__ __forceinline__ void spin_until_ge(const Watch& w, const int* p, int v) {
+    if (ld_acquire(p) >= v) return;
+    const unsigned long long t0 = global_ns();
+    for (unsigned it = 1; ld_acquire(p) < v; ++it) {
+        __nanosleep(64);
+        if ((it & 1023u) == 0u) wd_check(w, t0);
+    }
+}
+__device__ __forceinline__ void mbar_wait_wd(const Watch& w, uint64_t* bar, uint32_t parity) {
+    if (mbar_try_wait(bar, parity)) return;
+    const unsigned long long t0 = global_ns();
+    for (unsigned it = 1; !mbar_try_wait(bar, parity); ++it)
+        if ((it & 4095u) == 0u) wd_check(w, t0);
 }
 
 // shared memory of one CTA: workers use the column ring, the chain CTA the hand-off ring
@@ -143,32 +176,29 @@ template <int ROWS, bool UNIFORM>
 __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned& kring, int row0, int nrows,
                                           int cbeg, int gap0, int gap1, int v0, int v1) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    constexpr int kConsumerWarps = kBulkThreads / 32;
     const int gap = gap1 - gap0;
     const int gapv = gap0 - cbeg;
+    const Watch wd{p.sy, p.st};
 
-    if (warp == kConsumerWarps) {
-        if (lane == 0) {
-            fence_proxy_async();
-            unsigned k = kring;
-            for (int v = v0; v < v1; ++k) {
-                const int lim = (v < gapv) ? min(v1, gapv) : v1;
-                const int cnt = min(kColTile, lim - v);
-                const int a = cbeg + ((v < gapv) ? v : v + gap);
-                const unsigned s = k % kStages;
-                if (k >= (unsigned)kStages) mbar_wait(&sh.empty_bar[s], ((k / kStages) - 1) & 1);
-                mbar_arrive_expect_tx(&sh.full_bar[s], (uint32_t)cnt * (UNIFORM ? 32u : 40u));
-                bulk_g2s(sh.u.w.stage[s].xy, p.xy + a, (uint32_t)cnt * 16u, &sh.full_bar[s]);
-                bulk_g2s(sh.u.w.stage[s].zq, p.zq + a, (uint32_t)cnt * 16u, &sh.full_bar[s]);
-                if (!UNIFORM) bulk_g2s(sh.u.w.stage[s].h, p.hh + a, (uint32_t)cnt * 8u, &sh.full_bar[s]);
-                v += cnt;
-            }
-        }
-        for (int v = v0; v < v1; ++kring) {   // every thread advances the ring counter identically
-            const int lim = (v < gapv) ? min(v1, gapv) : v1;
-            v += min(kColTile, lim - v);
-        }
-        return;
+    // producer state (thread 0 only): next stage to issue
+    unsigned kp = kring;
+    int vp = v0;
+    auto issue = [&]() {
+        const int lim = (vp < gapv) ? min(v1, gapv) : v1;
+        const int cnt = min(kColTile, lim - vp);
+        const int a = cbeg + ((vp < gapv) ? vp : vp + gap);
+        const unsigned s = kp % kStages;
+        if (kp >= (unsigned)kStages) mbar_wait_wd(wd, &sh.empty_bar[s], ((kp / kStages) - 1) & 1);
+        mbar_arrive_expect_tx(&sh.full_bar[s], (uint32_t)cnt * (UNIFORM ? 32u : 40u));
+        bulk_g2s(sh.u.w.stage[s].xy, p.xy + a, (uint32_t)cnt * 16u, &sh.full_bar[s]);
+        bulk_g2s(sh.u.w.stage[s].zq, p.zq + a, (uint32_t)cnt * 16u, &sh.full_bar[s]);
+        if (!UNIFORM) bulk_g2s(sh.u.w.stage[s].h, p.hh + a, (uint32_t)cnt * 8u, &sh.full_bar[s]);
+        vp += cnt;
+        ++kp;
+    };
+    if (tid == 0) {
+        fence_proxy_async();
+        for (int q = 0; q < kStages - 1 && vp < v1; ++q) issue();
     }
 
     RowRegs R[ROWS];
@@ -193,7 +223,9 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
         const int lim = (v < gapv) ? min(v1, gapv) : v1;
         const int cnt = min(kColTile, lim - v);
         const unsigned s = k % kStages;
-        mbar_wait(&sh.full_bar[s], (k / kStages) & 1);
+        if (tid == 0 && vp < v1) issue();   // keeps kStages - 1 stages in flight ahead of this one
+        __syncwarp();
+        mbar_wait_wd(wd, &sh.full_bar[s], (k / kStages) & 1);
         const ColStage& st = sh.u.w.stage[s];
         if (warp_live) {
 #pragma unroll 1
@@ -247,6 +279,7 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
     const int slot = gt % kRing;
     HandOff& ho = sh.u.ho[slot];
     const unsigned apar = (unsigned)(c >> 1) & 1u;
+    const Watch wd{a.sy, a.p.st};
 
     // base sum of all FAR, FIX and DIAG items of this row
     double E = accum_value(__ldcg(a.p.S1 + i), __ldcg(a.p.S2 + i));
@@ -261,7 +294,7 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
     bool staged = false;
     auto stage_blocks = [&]() {
         // the slot is free once the publisher is done with tile gt - kRing
-        if (gt >= kRing) mbar_wait(&sh.p_bar[slot], (unsigned)(gt / kRing - 1) & 1u);
+        if (gt >= kRing) mbar_wait_wd(wd, &sh.p_bar[slot], (unsigned)(gt / kRing - 1) & 1u);
         if (lane == 0) {
             const double* src = B.Dblk + (size_t)blk_index(t, t > 0 ? t - 1 : 0) * (kTile * kTile);
             const uint32_t bytes = (t > 0 ? 2u : 1u) * kTile * kTile * 8u;
@@ -275,7 +308,7 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
     // corrections of the column tiles s <= t - 2, as their accept masks appear
     for (int s = 0; s + 2 <= t; ++s) {
         if (!staged && s + kRing >= t) stage_blocks();
-        mbar_wait(&sh.a_bar[c & 1][s], apar);
+        mbar_wait_wd(wd, &sh.a_bar[c & 1][s], apar);
         const unsigned A = sh.sA[c & 1][s];
         const double* blk = B.Dblk + (size_t)blk_index(t, s) * (kTile * kTile);
         double v[kTile];
@@ -306,13 +339,14 @@ __device__ __forceinline__ void chain_publisher(const PArgs& a, PShared& sh) {
     const int lane = threadIdx.x & 31;
     const Params& p = a.p;
     const int C = a.C, GPC = C / kGroup, ntfull = C / kTile;
+    const Watch wd{a.sy, a.p.st};
     unsigned long long n_acc = 0, n_ov = 0, n_wall = 0, n_tie = 0;
     double e_lane = 0.0;
     for (int c = 0; c < a.nchunks; ++c) {
         const int row0 = c * C, nt = chunk_rows(p.Np, C, c) / kTile;
         for (int t = 0; t < nt; ++t) {
             const int gt = c * ntfull + t, slot = gt % kRing;
-            mbar_wait(&sh.a_bar[c & 1][t], (unsigned)(c >> 1) & 1u);
+            mbar_wait_wd(wd, &sh.a_bar[c & 1][t], (unsigned)(c >> 1) & 1u);
             const HandOff& ho = sh.u.ho[slot];
             const int i = row0 + t * kTile + lane;
             const unsigned fl = ho.out_flags[lane];
@@ -375,6 +409,7 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
     const Params& p = a.p;
     const int C = a.C;
     const int ntfull = C / kTile;
+    const Watch wd{a.sy, a.p.st};
 
     if (warp == kHelpers + 1) {
         chain_publisher(a, sh);
@@ -388,10 +423,10 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
             if (h >= nt) continue;
             if (lane == 0) {
                 const long long t0 = clock64();
-                spin_until_ge(sy_far_done(a) + c, far_slices(far_cols(p.Np, C, c), a.farcols));
-                spin_until_ge(sy_diag_done(a) + c, diag_items(nrows));
+                spin_until_ge(wd, sy_far_done(a) + c, far_slices(far_cols(p.Np, C, c), a.farcols));
+                spin_until_ge(wd, sy_diag_done(a) + c, diag_items(nrows));
                 const long long t1 = clock64();
-                if (c > 0) spin_until_ge(sy_fix_done(a) + c, C / kFixCols);
+                if (c > 0) spin_until_ge(wd, sy_fix_done(a) + c, C / kFixCols);
                 if (h == 0 && a.dbg) { a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t1; }
             }
             __syncwarp();
@@ -410,7 +445,7 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
         for (int t = 0; t < nt; ++t) {
             const int gt = c * ntfull + t, slot = gt % kRing;
             const long long tw = clock64();
-            mbar_wait(&sh.ho_bar[slot], (unsigned)(gt / kRing) & 1u);
+            mbar_wait_wd(wd, &sh.ho_bar[slot], (unsigned)(gt / kRing) & 1u);
             if (t == 0) w_first += clock64() - tw; else w_other += clock64() - tw;
             HandOff& ho = sh.u.ho[slot];
             const double lbq = ho.lbq[lane], lnu = ho.lnu[lane];
@@ -514,7 +549,9 @@ __device__ __forceinline__ void fetch_item(const PArgs& a, Cursor& cfar, Cursor&
     const int C = a.C, GPC = C / kGroup, fix_per_chunk = C / kFixCols;
     const int total_urgent = (a.nchunks - 1) * fix_per_chunk;
     int* sy = a.sy;
-    for (;;) {
+    const Watch wd{a.sy, a.p.st};
+    for (unsigned it = 1;; ++it) {
+        if ((it & 1023u) == 0u) wd_check(wd, global_ns());   // no time limit of its own: leaves when another wait gave up
         bool far_done = true, diag_done = false;
         if (cdiag.ticket >= 0 && try_queue<false>(a, cdiag, item, diag_done)) return;
         if (!near && try_queue<true>(a, cfar, item, far_done)) return;
@@ -547,7 +584,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) {
             mbar_init(&sh.full_bar[s], 1);
-            mbar_init(&sh.empty_bar[s], kBulkThreads / 32);
+            mbar_init(&sh.empty_bar[s], kPThreads / 32);
         }
         for (int s = 0; s < kRing; ++s) { mbar_init(&sh.ho_bar[s], 2); mbar_init(&sh.p_bar[s], 1); }
         for (int s = 0; s < 2 * (kChunkMax / kTile); ++s) mbar_init(&sh.a_bar[0][0] + s, 1);
@@ -560,7 +597,12 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
             st_release(a.sy + kSyChainSm, (int)smid + 1);
         } else {
             int v;
-            while ((v = ld_acquire(a.sy + kSyChainSm)) == 0) __nanosleep(100);
+            const Watch wd{a.sy, a.p.st};
+            const unsigned long long t0 = global_ns();
+            for (unsigned it = 1; (v = ld_acquire(a.sy + kSyChainSm)) == 0; ++it) {
+                __nanosleep(100);
+                if ((it & 1023u) == 0u) wd_check(wd, t0);
+            }
             sh.item[0] = (v == (int)smid + 1) ? 1 : 0;
         }
     }
@@ -582,10 +624,12 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
             if (a.dbg) {
                 atomicAdd((unsigned long long*)a.dbg + 5, (unsigned long long)(clock64() - t0));
                 atomicAdd((unsigned long long*)a.dbg + 6 + sh.item[0], 1ull);   // [6] exits, [7] diag, [8] far, [9] fix
+                if (sh.item[0] == kItemFar) ((volatile int*)(a.dbg + 16))[300 + blockIdx.x] += 1;
             }
         }
         __syncthreads();
         const int type = sh.item[0], c = sh.item[1], k = sh.item[2];
+        if (a.dbg && tid == 0) ((volatile int*)(a.dbg + 16))[blockIdx.x] = (type << 28) | (c << 16) | k;
         if (type == kItemExit) break;
         const int row0 = c * C, nrows = chunk_rows(p.Np, C, c);
         int* counter;
@@ -611,10 +655,16 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
             bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, cb, cb, 0, kFixCols);
             counter = sy_fix_done(a) + c;
         }
+        (void)counter;
         __syncthreads();
         if (tid == 0) {
+            // completion counter of this item's queue and chunk (item[] is stable until the next fetch)
+            const int ty = ((volatile int*)sh.item)[0], cc = ((volatile int*)sh.item)[1];
+            int* done = (ty == kItemFar ? sy_far_done(a) : ty == kItemDiag ? sy_diag_done(a) : sy_fix_done(a)) + cc;
             __threadfence();
-            atomicAdd(counter, 1);
+            atomicAdd(done, 1);
+            if (a.dbg) ((volatile int*)(a.dbg + 16))[blockIdx.x] = 0;
+            if (a.dbg) ((volatile int*)(a.dbg + 16))[600 + blockIdx.x] += 1;
         }
     }
 }
