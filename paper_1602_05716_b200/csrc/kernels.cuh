@@ -58,7 +58,7 @@ __device__ __forceinline__ double accum_value(long long s1, long long s2) {
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_trial(Params p) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < p.sy_n) p.sy[i] = 0;
+    for (int j = i; j < p.sy_n; j += gridDim.x * blockDim.x) p.sy[j] = 0;
     if (i >= p.Np) return;
     p.S1[i] = 0ll; p.S2[i] = 0ll; p.ovc[i] = 0;
     const double2 xy = p.xy[i];
@@ -318,6 +318,7 @@ __device__ __forceinline__ void diag_unit(const Params& p, int row0, int nrows, 
     int ovc = 0;
     unsigned ovo = 0u, ovn = 0u;
     double* blk = (s <= t) ? p.Dblk + (size_t)blk_index(t, s) * (kTile * kTile) : nullptr;
+#pragma unroll 4
     for (int jj = 0; jj < kTile; ++jj) {
         const double2 a = cxy[jj];
         const double2 b = czq[jj];

@@ -56,7 +56,7 @@ Layout make_layout(int64_t N) {
     take(65536);
     L.sy = take((size_t)(kSyHdr + 4 * (Np / 256 + 1)) * 4);
     take(65536);
-    L.dbg = take(16 * 8 + 2048 * 4);
+    L.dbg = take(16 * 8 + 1024 * 8);
     L.log_dE = take(Np * 8); L.log_flags = take(Np);
     L.st = take(sizeof(DevState));
     L.epart = take((size_t)kEnergySlices * Np * 8 + 8);
@@ -83,6 +83,8 @@ struct mc_handle {
     int engine = 1;          // 1: one persistent kernel per sweep (persist.cuh); 0: kernels per chunk in a graph
     int prows = 4;           // rows per consumer thread of the persistent kernel (chunk = 256 * prows)
     int pfarcols = 128;      // columns per FAR item of the persistent kernel
+    int pmode = 0;           // 1: throughput probe (diagnostic; the sweep's results are meaningless)
+    bool pwave = true;       // round the FAR items of a chunk to a multiple of the FAR workers
     int pnear = 16;          // worker CTAs of the persistent kernel that serve FIX and DIAG items only
     bool debug = false;      // collect the cycle counters of mc_debug_counters
     int pgrid = 0;           // CTAs of the persistent kernel (0: not yet configured)
@@ -251,10 +253,12 @@ int launch_sweep_kernel(mc_handle* h, cudaStream_t s) {
     a.nchunks = (a.p.Np + a.C - 1) / a.C;
     a.nnear = std::min(h->pnear, std::max(0, h->pgrid - 4));
     a.farcols = h->pfarcols;
+    a.mode = h->pmode;
+    a.nfar = h->pwave ? std::max(1, h->pgrid - 2 - a.nnear) : 0;
     a.sy = h->p.sy;
     char* w = h->ws;
     a.dbg = h->debug ? (long long*)(w + h->L.dbg) : nullptr;
-    if (a.dbg) CUDA_TRY(cudaMemsetAsync(a.dbg, 0, 16 * 8, s));
+    if (a.dbg) CUDA_TRY(cudaMemsetAsync(a.dbg, 0, 16 * 8 + 1024 * 8, s));
     void* args[] = {(void*)&a};
     CUDA_TRY(cudaLaunchCooperativeKernel((void*)kern, dim3(h->pgrid), dim3(kPThreads), args, (size_t)smem, s));
     return MC_OK;
@@ -362,7 +366,7 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     p.st = (DevState*)(w + L.st);
     p.sy = (int*)(w + L.sy);
     p.S1 = (long long*)(w + L.S1); p.S2 = (long long*)(w + L.S2); p.ovc = (int*)(w + L.ovc);
-    p.sy_n = kSyHdr + 4 * (p.Np / 256 + 1);
+    p.sy_n = kSyHdr + 4 * (p.Np / 256 + 1);   // header + per-chunk counters
     h->prows = p.Np >= 16384 ? 4 : (p.Np >= 2048 ? 2 : 1);
     p.R = cavity_R; p.lB = bjerrum_length; p.max_disp = max_disp; p.seed = seed;
     h->epart = (double*)(w + L.epart);
@@ -644,6 +648,10 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     } else if (!std::strcmp(key, "far_cols")) {
         if (value < 8 || value > 65536 || value % 8) return fail(MC_EINVAL, "far_cols must be a multiple of 8 in 8..65536");
         h->pfarcols = (int)value;
+    } else if (!std::strcmp(key, "probe")) {
+        h->pmode = value != 0 ? 1 : 0;
+    } else if (!std::strcmp(key, "wave")) {
+        h->pwave = value != 0;
     } else if (!std::strcmp(key, "pnear")) {
         if (value < 0 || value > 128) return fail(MC_EINVAL, "pnear must be in 0..128");
         h->pnear = (int)value;

@@ -28,7 +28,9 @@ constexpr int kRing = 4;                       // hand-off ring depth of the cha
 constexpr int kHelpers = 6;
 
 // scheduling state in global memory; zeroed by k_trial at the start of every sweep
-enum { kSyTicket = 0, kSyUTicket = 1, kSyGroups = 2, kSyChainSm = 3, kSyDTicket = 4, kSyAbort = 5, kSyHdr = 8 };
+// (hot words 128 bytes apart, so that polling one does not slow down atomics on another)
+enum { kSyTicket = 0, kSyUTicket = 32, kSyGroups = 64, kSyChainSm = 96, kSyDTicket = 128, kSyAbort = 160, kSyTicketU = 192,
+       kSyHdr = 256 };
 
 struct PArgs {
     Params p;
@@ -36,16 +38,30 @@ struct PArgs {
     int nchunks;
     int farcols;      // target columns per FAR item (multiple of 8)
     int nnear;        // worker CTAs 1..nnear serve FIX and DIAG only
+    int nfar;         // number of FAR workers (0: do not round item counts to it)
+    int mode;         // 0 normal; 1 throughput probe: no chain, every CTA runs QU items over all columns but the chunk's own
     int* sy;          // [kSyHdr + 3 * nchunks]: header, far_done, diag_done, fix_done
     long long* dbg;   // [16] diagnostic cycle counters (see mc_debug_counters), may be null
 };
 
 __host__ __device__ inline int chunk_rows(int Np, int C, int c) { return min(C, Np - c * C); }
-__host__ __device__ inline int far_cols(int Np, int C, int c) {
-    const int row0 = c * C, prev0 = c > 0 ? row0 - C : row0;
-    return Np - (row0 + chunk_rows(Np, C, c) - prev0);
+// FAR items of one chunk over ncols columns: about farcols columns each, and -- when there are at
+// least half as many as FAR workers -- a whole number of items per worker, so that a wave of items
+// ends for all workers at about the same time
+__host__ __device__ inline int far_slices(int ncols, int farcols, int nfar) {
+    int n = (ncols + farcols - 1) / farcols;
+    if (nfar > 0 && 2 * n >= nfar) n = ((2 * n + nfar) / (2 * nfar)) * nfar;   // nearest multiple, at least one
+    if (n > ncols / 8) n = ncols / 8;
+    return n;
 }
-__host__ __device__ inline int far_slices(int ncols, int farcols) { return (ncols + farcols - 1) / farcols; }
+// columns of the FAR items of chunk c: L = before chunk c-1 (final positions once the chain has
+// finished chunk c-2), U = after chunk c (sweep-start positions, never blocked)
+__host__ __device__ inline int farL_cols(int C, int c) { return c >= 2 ? (c - 1) * C : 0; }
+__host__ __device__ inline int farU_cols(int Np, int C, int c) { return Np - (c * C + chunk_rows(Np, C, c)); }
+__host__ __device__ inline int probe_cols(int Np, int C, int c) { return Np - chunk_rows(Np, C, c); }
+__host__ __device__ inline int far_items(int Np, int C, int farcols, int nfar, int c) {
+    return far_slices(farL_cols(C, c), farcols, nfar) + far_slices(farU_cols(Np, C, c), farcols, nfar);
+}
 __host__ __device__ inline int diag_items(int nrows) {
     const int nt = nrows / kTile;
     return (nt * nt + 7) / 8;
@@ -423,11 +439,14 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
             if (h >= nt) continue;
             if (lane == 0) {
                 const long long t0 = clock64();
-                spin_until_ge(wd, sy_far_done(a) + c, far_slices(far_cols(p.Np, C, c), a.farcols));
+                spin_until_ge(wd, sy_far_done(a) + c, far_items(p.Np, C, a.farcols, a.nfar, c));
                 spin_until_ge(wd, sy_diag_done(a) + c, diag_items(nrows));
                 const long long t1 = clock64();
                 if (c > 0) spin_until_ge(wd, sy_fix_done(a) + c, C / kFixCols);
-                if (h == 0 && a.dbg) { a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t1; }
+                if (h == 0 && a.dbg) {
+                    a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t1;
+                    if (c < 300) a.dbg[16 + 3 * c] = (long long)global_ns();   // inputs of chunk c complete
+                }
             }
             __syncwarp();
             const ChunkBufs B = chunk_bufs(a, c);
@@ -447,6 +466,7 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
             const long long tw = clock64();
             mbar_wait_wd(wd, &sh.ho_bar[slot], (unsigned)(gt / kRing) & 1u);
             if (t == 0) w_first += clock64() - tw; else w_other += clock64() - tw;
+            if (t == 0 && lane == 0 && a.dbg && c < 300) a.dbg[16 + 3 * c + 1] = (long long)global_ns();   // chain starts chunk c
             HandOff& ho = sh.u.ho[slot];
             const double lbq = ho.lbq[lane], lnu = ho.lnu[lane];
             double Eu = ho.E[lane];
@@ -493,6 +513,7 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&sh.a_bar[c & 1][t]);
         }
+        if (lane == 0 && a.dbg && c < 300) a.dbg[16 + 3 * c + 2] = (long long)global_ns();   // chain ends chunk c
     }
     if (lane == 0 && a.dbg) {
         a.dbg[0] = clock64() - t_start;   // chain warp: whole sweep
@@ -505,71 +526,114 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
 
 namespace mcb {
 
-enum { kItemExit = 0, kItemDiag = 1, kItemFar = 2, kItemFix = 3 };
+enum { kItemExit = 0, kItemDiag = 1, kItemFarL = 2, kItemFix = 3, kItemFarU = 4 };
 
-// Thread 0 of a worker CTA claims the next item.  Three queues, each a ticket counter in global
-// memory: FIX (urgent; an item exists once the chain has published its columns), DIAG and FAR (in
-// chunk order; chunk c is released when the chain has finished chunk c-2).  "Near" workers (the
-// first a.nnear worker CTAs) serve FIX and DIAG only, so that the chain never waits for a CTA that
-// is busy with a long FAR item; the others serve FAR and help with FIX/DIAG whenever their FAR
-// ticket is not released yet.  A claimed ticket is kept until it is released, and a held DIAG
-// ticket goes before FAR: every item the chain can be waiting for is then either claimed by a
-// CTA that will run it next, or still claimable.
+// Work queues.  Each is a ticket counter in global memory; tickets run through the chunks in order.
+//   QL  FAR items over the columns before chunk c-1 (final positions): released when the chain
+//       has finished chunk c-2
+//   QU  FAR items over the columns after chunk c (sweep-start positions): never blocked -- the
+//       filler that keeps every SM busy while the chain works
+//   QD  DIAG items: released with QL (the D buffers are double-buffered by chunk parity)
+//   FIX urgent items: exist as soon as the chain has published their 16 columns
+// Thread 0 of a worker CTA reads all five words (four counters and the chain's progress) in one
+// round trip, picks the first queue whose next ticket is released -- QL, FIX, QD, QU for the FAR
+// workers; FIX, QD for the a.nnear "near" workers that keep the latency of what the chain waits
+// for short -- and claims with one atomic.  A ticket is claimed only when its chunk is released
+// (a claim that races across a chunk boundary into an unreleased chunk is kept and run first once
+// released), so no CTA sits on work that another CTA could do.
+enum { QL = 0, QU = 1, QD = 2 };
 struct Cursor {
-    int ticket;     // claimed ticket, -1 if none
-    int c, base;    // chunk the cursor is in, first ticket of that chunk
+    int c, base;    // chunk that holds the queue's next ticket, first ticket of that chunk
+    int held;       // ticket claimed at a chunk boundary before its chunk was released (-1: none)
+};
+struct Cursors {
+    Cursor l, u, d;
 };
 
-template <bool FAR>
+template <int Q>
 __device__ __forceinline__ int items_of(const PArgs& a, int c) {
-    return FAR ? far_slices(far_cols(a.p.Np, a.C, c), a.farcols) : diag_items(chunk_rows(a.p.Np, a.C, c));
+    return Q == QL ? far_slices(farL_cols(a.C, c), a.farcols, a.nfar)
+         : Q == QU ? far_slices(a.mode == 1 ? probe_cols(a.p.Np, a.C, c) : farU_cols(a.p.Np, a.C, c), a.farcols, a.nfar)
+                   : diag_items(chunk_rows(a.p.Np, a.C, c));
+}
+template <int Q>
+__device__ __forceinline__ void advance(const PArgs& a, Cursor& cur, int t) {
+    while (cur.c < a.nchunks && t >= cur.base + items_of<Q>(a, cur.c)) {
+        cur.base += items_of<Q>(a, cur.c);
+        ++cur.c;
+    }
+}
+__device__ __forceinline__ bool released(const PArgs& a, int c, int groups) {
+    return c < 2 || groups >= (c - 1) * (a.C / kGroup);
 }
 
-// true if an item of this queue was taken (written to item[]); done = queue exhausted
-template <bool FAR>
-__device__ __forceinline__ bool try_queue(const PArgs& a, Cursor& cur, int* item, bool& done) {
-    if (cur.ticket < 0 && cur.c < a.nchunks) {
-        cur.ticket = atomicAdd(a.sy + (FAR ? kSyTicket : kSyDTicket), 1);
-        while (cur.c < a.nchunks && cur.ticket >= cur.base + items_of<FAR>(a, cur.c)) {
-            cur.base += items_of<FAR>(a, cur.c);
-            ++cur.c;
-        }
+// t = the counter's value as just read, groups = the chain's progress as just read.
+// true if an item of queue Q was claimed (written to item[]); done = queue exhausted
+template <int Q>
+__device__ __forceinline__ bool try_queue(const PArgs& a, Cursor& cur, int t, int groups, int* item, bool& done) {
+    int* counter = a.sy + (Q == QL ? kSyTicket : Q == QU ? kSyTicketU : kSyDTicket);
+    int mine = cur.held;
+    if (mine < 0) {
+        advance<Q>(a, cur, t);
+        done = cur.c >= a.nchunks;
+        if (done || (Q != QU && !released(a, cur.c, groups))) return false;
+        mine = atomicAdd(counter, 1);
+        advance<Q>(a, cur, mine);
+        done = cur.c >= a.nchunks;
+        if (done) return false;
     }
-    done = cur.c >= a.nchunks;
-    if (done) return false;
-    if (cur.c >= 2 && ld_acquire(a.sy + kSyGroups) < (cur.c - 1) * (a.C / kGroup)) return false;
-    item[0] = FAR ? kItemFar : kItemDiag;
+    done = false;
+    if (Q != QU && !released(a, cur.c, groups)) {
+        cur.held = mine;
+        return false;
+    }
+    cur.held = -1;
+    item[0] = Q == QL ? kItemFarL : Q == QU ? kItemFarU : kItemDiag;
     item[1] = cur.c;
-    item[2] = cur.ticket - cur.base;
-    cur.ticket = -1;
+    item[2] = mine - cur.base;
     return true;
 }
 
-__device__ __forceinline__ void fetch_item(const PArgs& a, Cursor& cfar, Cursor& cdiag, bool near, int* item) {
+__device__ __forceinline__ int ld_relaxed(const int* p) {
+    int v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near, int* item) {
     const int C = a.C, GPC = C / kGroup, fix_per_chunk = C / kFixCols;
     const int total_urgent = (a.nchunks - 1) * fix_per_chunk;
     int* sy = a.sy;
     const Watch wd{a.sy, a.p.st};
     for (unsigned it = 1;; ++it) {
         if ((it & 1023u) == 0u) wd_check(wd, global_ns());   // no time limit of its own: leaves when another wait gave up
-        bool far_done = true, diag_done = false;
-        if (cdiag.ticket >= 0 && try_queue<false>(a, cdiag, item, diag_done)) return;
-        if (!near && try_queue<true>(a, cfar, item, far_done)) return;
-        const int u = *(volatile int*)(sy + kSyUTicket);
-        if (u < total_urgent) {
+        // one round trip: five independent loads
+        const int tl = ld_relaxed(sy + kSyTicket), tu = ld_relaxed(sy + kSyTicketU), td = ld_relaxed(sy + kSyDTicket);
+        const int u = ld_relaxed(sy + kSyUTicket), groups = ld_relaxed(sy + kSyGroups);
+        bool got = false, l_done = true, u_done = true, d_done = false;
+        if (a.mode == 1) {
+            got = try_queue<QU>(a, cur.u, tu, groups, item, u_done);
+            if (!got) item[0] = kItemExit;
+            return;
+        }
+        if (!near) got = try_queue<QL>(a, cur.l, tl, groups, item, l_done);
+        if (!got && u < total_urgent) {
             const int c = 1 + u / fix_per_chunk, j = u % fix_per_chunk;
             const int need = (c - 1) * GPC + (j * kFixCols) / kGroup + 1;
-            if (ld_acquire(sy + kSyGroups) >= need) {
-                if (atomicCAS(sy + kSyUTicket, u, u + 1) == u) {
-                    item[0] = kItemFix; item[1] = c; item[2] = j;
-                    return;
-                }
-                continue;
+            if (groups >= need) {
+                if (atomicCAS(sy + kSyUTicket, u, u + 1) != u) continue;
+                item[0] = kItemFix; item[1] = c; item[2] = j;
+                got = true;
             }
         }
-        if (try_queue<false>(a, cdiag, item, diag_done)) return;
-        if (far_done && diag_done && u >= total_urgent) { item[0] = kItemExit; return; }
-        __nanosleep(100);
+        if (!got) got = try_queue<QD>(a, cur.d, td, groups, item, d_done);
+        if (!got && !near) got = try_queue<QU>(a, cur.u, tu, groups, item, u_done);
+        if (got) {
+            __threadfence();   // acquire: what the chain published before the progress value read above
+            return;
+        }
+        if (l_done && u_done && d_done && u >= total_urgent) { item[0] = kItemExit; return; }
+        __nanosleep(near ? 400 : 200);
     }
 }
 
@@ -607,29 +671,28 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
         }
     }
     __syncthreads();
-    if (blockIdx.x == 0) {
+    if (blockIdx.x == 0 && a.mode != 1) {
         chain_cta(a, sh);
         return;
     }
-    if (sh.item[0] == 1) return;
+    if (sh.item[0] == 1 && a.mode != 1) return;
 
-    Cursor cfar{-1, 0, 0}, cdiag{-1, 0, 0};
+    Cursors cur{{0, 0, -1}, {0, 0, -1}, {0, 0, -1}};
     const bool near = (int)blockIdx.x <= a.nnear;
     unsigned kring = 0;
     for (;;) {
         __syncthreads();
         if (tid == 0) {
             const long long t0 = clock64();
-            fetch_item(a, cfar, cdiag, near, sh.item);
+            fetch_item(a, cur, near, sh.item);
             if (a.dbg) {
                 atomicAdd((unsigned long long*)a.dbg + 5, (unsigned long long)(clock64() - t0));
-                atomicAdd((unsigned long long*)a.dbg + 6 + sh.item[0], 1ull);   // [6] exits, [7] diag, [8] far, [9] fix
-                if (sh.item[0] == kItemFar) ((volatile int*)(a.dbg + 16))[300 + blockIdx.x] += 1;
+                atomicAdd((unsigned long long*)a.dbg + 6 + sh.item[0], 1ull);   // [6] exits, [7] diag, [8] farL, [9] fix, [10] farU
             }
         }
         __syncthreads();
         const int type = sh.item[0], c = sh.item[1], k = sh.item[2];
-        if (a.dbg && tid == 0) ((volatile int*)(a.dbg + 16))[blockIdx.x] = (type << 28) | (c << 16) | k;
+        const long long t_item = clock64();
         if (type == kItemExit) break;
         const int row0 = c * C, nrows = chunk_rows(p.Np, C, c);
         int* counter;
@@ -643,12 +706,14 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
                                 sh.u.w.ch[warp], sh.u.w.ctz[warp]);
             }
             counter = sy_diag_done(a) + c;
-        } else if (type == kItemFar) {
-            const int prev0 = c > 0 ? row0 - C : row0;
-            const int ncols = far_cols(p.Np, C, c);
-            const int nf = far_slices(ncols, a.farcols);
+        } else if (type == kItemFarL || type == kItemFarU) {
+            // columns [cb, cb + ncols): before chunk c-1 (L) or after chunk c (U); probe: all but the chunk's own
+            const bool probe = a.mode == 1;
+            const int cb = (type == kItemFarL || probe) ? 0 : row0 + nrows;
+            const int ncols = probe ? probe_cols(p.Np, C, c) : type == kItemFarL ? farL_cols(C, c) : farU_cols(p.Np, C, c);
+            const int nf = far_slices(ncols, a.farcols, a.nfar);
             const int v0 = slice_bound(ncols, nf, k), v1 = slice_bound(ncols, nf, k + 1);
-            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, 0, prev0, row0 + nrows, v0, v1);
+            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, probe ? row0 : cb, probe ? row0 + nrows : cb, v0, v1);
             counter = sy_far_done(a) + c;
         } else {
             const int cb = row0 - C + k * kFixCols;
@@ -660,11 +725,14 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
         if (tid == 0) {
             // completion counter of this item's queue and chunk (item[] is stable until the next fetch)
             const int ty = ((volatile int*)sh.item)[0], cc = ((volatile int*)sh.item)[1];
-            int* done = (ty == kItemFar ? sy_far_done(a) : ty == kItemDiag ? sy_diag_done(a) : sy_fix_done(a)) + cc;
+            int* done = (ty == kItemDiag ? sy_diag_done(a) : ty == kItemFix ? sy_fix_done(a) : sy_far_done(a)) + cc;
             __threadfence();
             atomicAdd(done, 1);
-            if (a.dbg) ((volatile int*)(a.dbg + 16))[blockIdx.x] = 0;
-            if (a.dbg) ((volatile int*)(a.dbg + 16))[600 + blockIdx.x] += 1;
+            if (a.dbg) {
+                const unsigned long long dt = (unsigned long long)(clock64() - t_item);
+                atomicAdd((unsigned long long*)a.dbg + 10 + (ty == kItemFarU ? kItemFarL : ty), dt);   // busy cycles: [11] diag [12] far [13] fix
+                if (near) atomicAdd((unsigned long long*)a.dbg + 14, dt);                              // [14] near workers
+            }
         }
     }
 }
