@@ -23,7 +23,8 @@ namespace mcb {
 
 constexpr int kPThreads = kBulkThreads;        // workers: 8 consumer warps; thread 0 also feeds the column ring
 constexpr int kGroup = 128;                    // rows per published progress step of the chain
-constexpr int kFixCols = 16;                   // columns per FIX item
+constexpr int kFixCols = 16;                   // columns per FIX item (columns of chunk c-1)
+constexpr int kMidCols = 32;                   // columns per MID item (columns of chunk c-2)
 constexpr int kRing = 4;                       // hand-off ring depth of the chain CTA
 constexpr int kHelpers = 6;
 
@@ -54,9 +55,13 @@ __host__ __device__ inline int far_slices(int ncols, int farcols, int nfar) {
     if (n > ncols / 8) n = ncols / 8;
     return n;
 }
-// columns of the FAR items of chunk c: L = before chunk c-1 (final positions once the chain has
-// finished chunk c-2), U = after chunk c (sweep-start positions, never blocked)
-__host__ __device__ inline int farL_cols(int C, int c) { return c >= 2 ? (c - 1) * C : 0; }
+// columns of the FAR items of chunk c: L = before chunk c-2 (final positions once the chain has
+// finished chunk c-3), U = after chunk c (sweep-start positions, never blocked)
+__host__ __device__ inline int farL_cols(int C, int c) { return c >= 3 ? (c - 2) * C : 0; }
+// urgent items of chunk c: MID (columns of chunk c-2, c >= 2) then FIX (columns of chunk c-1, c >= 1)
+__host__ __device__ inline int urgent_items(int C, int c) {
+    return (c >= 2 ? C / kMidCols : 0) + (c >= 1 ? C / kFixCols : 0);
+}
 __host__ __device__ inline int farU_cols(int Np, int C, int c) { return Np - (c * C + chunk_rows(Np, C, c)); }
 __host__ __device__ inline int probe_cols(int Np, int C, int c) { return Np - chunk_rows(Np, C, c); }
 __host__ __device__ inline int far_items(int Np, int C, int farcols, int nfar, int c) {
@@ -440,11 +445,12 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
             if (lane == 0) {
                 const long long t0 = clock64();
                 spin_until_ge(wd, sy_far_done(a) + c, far_items(p.Np, C, a.farcols, a.nfar, c));
-                spin_until_ge(wd, sy_diag_done(a) + c, diag_items(nrows));
                 const long long t1 = clock64();
-                if (c > 0) spin_until_ge(wd, sy_fix_done(a) + c, C / kFixCols);
+                spin_until_ge(wd, sy_diag_done(a) + c, diag_items(nrows));
+                const long long t2 = clock64();
+                if (c > 0) spin_until_ge(wd, sy_fix_done(a) + c, urgent_items(C, c));
                 if (h == 0 && a.dbg) {
-                    a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t1;
+                    a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t2; a.dbg[15] += t2 - t1;
                     if (c < 300) a.dbg[16 + 3 * c] = (long long)global_ns();   // inputs of chunk c complete
                 }
             }
@@ -526,7 +532,7 @@ __device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
 
 namespace mcb {
 
-enum { kItemExit = 0, kItemDiag = 1, kItemFarL = 2, kItemFix = 3, kItemFarU = 4 };
+enum { kItemExit = 0, kItemDiag = 1, kItemFarL = 2, kItemFix = 3, kItemFarU = 4, kItemMid = 5 };
 
 // Work queues.  Each is a ticket counter in global memory; tickets run through the chunks in order.
 //   QL  FAR items over the columns before chunk c-1 (final positions): released when the chain
@@ -536,9 +542,9 @@ enum { kItemExit = 0, kItemDiag = 1, kItemFarL = 2, kItemFix = 3, kItemFarU = 4 
 //   QD  DIAG items: released with QL (the D buffers are double-buffered by chunk parity)
 //   FIX urgent items: exist as soon as the chain has published their 16 columns
 // Thread 0 of a worker CTA reads all five words (four counters and the chain's progress) in one
-// round trip, picks the first queue whose next ticket is released -- QL, FIX, QD, QU for the FAR
-// workers; FIX, QD for the a.nnear "near" workers that keep the latency of what the chain waits
-// for short -- and claims with one atomic.  A ticket is claimed only when its chunk is released
+// round trip, picks the first queue whose next ticket is released -- FIX/MID, QD, QL, QU for the
+// FAR workers (what the chain needs soonest first); FIX/MID, QD for the a.nnear "near" workers that
+// keep the latency of what the chain waits for short -- and claims with one atomic.  A ticket is claimed only when its chunk is released
 // (a claim that races across a chunk boundary into an unreleased chunk is kept and run first once
 // released), so no CTA sits on work that another CTA could do.
 enum { QL = 0, QU = 1, QD = 2 };
@@ -563,8 +569,10 @@ __device__ __forceinline__ void advance(const PArgs& a, Cursor& cur, int t) {
         ++cur.c;
     }
 }
+// QL items of chunk c need the chain to have finished chunk c-3, QD items chunk c-2 (buffer parity)
+template <int Q>
 __device__ __forceinline__ bool released(const PArgs& a, int c, int groups) {
-    return c < 2 || groups >= (c - 1) * (a.C / kGroup);
+    return Q == QL ? (c < 3 || groups >= (c - 2) * (a.C / kGroup)) : (c < 2 || groups >= (c - 1) * (a.C / kGroup));
 }
 
 // t = the counter's value as just read, groups = the chain's progress as just read.
@@ -576,14 +584,14 @@ __device__ __forceinline__ bool try_queue(const PArgs& a, Cursor& cur, int t, in
     if (mine < 0) {
         advance<Q>(a, cur, t);
         done = cur.c >= a.nchunks;
-        if (done || (Q != QU && !released(a, cur.c, groups))) return false;
+        if (done || (Q != QU && !released<Q>(a, cur.c, groups))) return false;
         mine = atomicAdd(counter, 1);
         advance<Q>(a, cur, mine);
         done = cur.c >= a.nchunks;
         if (done) return false;
     }
     done = false;
-    if (Q != QU && !released(a, cur.c, groups)) {
+    if (Q != QU && !released<Q>(a, cur.c, groups)) {
         cur.held = mine;
         return false;
     }
@@ -601,8 +609,8 @@ __device__ __forceinline__ int ld_relaxed(const int* p) {
 }
 
 __device__ __forceinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near, int* item) {
-    const int C = a.C, GPC = C / kGroup, fix_per_chunk = C / kFixCols;
-    const int total_urgent = (a.nchunks - 1) * fix_per_chunk;
+    const int C = a.C, GPC = C / kGroup, nfix = C / kFixCols, nmid = C / kMidCols;
+    const int total_urgent = a.nchunks >= 2 ? nfix + (a.nchunks - 2) * (nfix + nmid) : 0;
     int* sy = a.sy;
     const Watch wd{a.sy, a.p.st};
     for (unsigned it = 1;; ++it) {
@@ -616,17 +624,24 @@ __device__ __forceinline__ void fetch_item(const PArgs& a, Cursors& cur, bool ne
             if (!got) item[0] = kItemExit;
             return;
         }
-        if (!near) got = try_queue<QL>(a, cur.l, tl, groups, item, l_done);
         if (!got && u < total_urgent) {
-            const int c = 1 + u / fix_per_chunk, j = u % fix_per_chunk;
-            const int need = (c - 1) * GPC + (j * kFixCols) / kGroup + 1;
+            // urgent ticket u -> chunk c, MID item j (columns of chunk c-2) or FIX item j (columns of chunk c-1)
+            int c = 1, j = u, mid = 0;
+            if (u >= nfix) {
+                c = 2 + (u - nfix) / (nfix + nmid);
+                j = (u - nfix) % (nfix + nmid);
+                mid = j < nmid ? 1 : 0;
+                if (!mid) j -= nmid;
+            }
+            const int need = mid ? (c - 1) * GPC : (c - 1) * GPC + (j * kFixCols) / kGroup + 1;
             if (groups >= need) {
                 if (atomicCAS(sy + kSyUTicket, u, u + 1) != u) continue;
-                item[0] = kItemFix; item[1] = c; item[2] = j;
+                item[0] = mid ? kItemMid : kItemFix; item[1] = c; item[2] = j;
                 got = true;
             }
         }
         if (!got) got = try_queue<QD>(a, cur.d, td, groups, item, d_done);
+        if (!got && !near) got = try_queue<QL>(a, cur.l, tl, groups, item, l_done);
         if (!got && !near) got = try_queue<QU>(a, cur.u, tu, groups, item, u_done);
         if (got) {
             __threadfence();   // acquire: what the chain published before the progress value read above
@@ -678,6 +693,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
     if (sh.item[0] == 1 && a.mode != 1) return;
 
     Cursors cur{{0, 0, -1}, {0, 0, -1}, {0, 0, -1}};
+    if (a.dbg && blockIdx.x == 1 && tid == 0) a.dbg[16 + 3 * 300 + 40] = (long long)global_ns();
     const bool near = (int)blockIdx.x <= a.nnear;
     unsigned kring = 0;
     for (;;) {
@@ -687,7 +703,12 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
             fetch_item(a, cur, near, sh.item);
             if (a.dbg) {
                 atomicAdd((unsigned long long*)a.dbg + 5, (unsigned long long)(clock64() - t0));
-                atomicAdd((unsigned long long*)a.dbg + 6 + sh.item[0], 1ull);   // [6] exits, [7] diag, [8] farL, [9] fix, [10] farU
+                if (!near) {   // FAR workers' fetch time by 0.5 ms bucket since the first chunk's start
+                    const long long origin = *(volatile long long*)(a.dbg + 16 + 3 * 300 + 40);
+                    const int bkt = origin ? (int)min(31ull, (global_ns() - (unsigned long long)origin) / 500000ull) : 0;
+                    atomicAdd((unsigned long long*)a.dbg + 16 + 3 * 300 + bkt, (unsigned long long)(clock64() - t0));
+                }
+                atomicAdd((unsigned long long*)a.dbg + 6 + (sh.item[0] == kItemMid ? kItemFix : sh.item[0]), 1ull);   // [6] exits, [7] diag, [8] farL, [9] fix, [10] farU
             }
         }
         __syncthreads();
@@ -715,6 +736,10 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
             const int v0 = slice_bound(ncols, nf, k), v1 = slice_bound(ncols, nf, k + 1);
             bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, probe ? row0 : cb, probe ? row0 + nrows : cb, v0, v1);
             counter = sy_far_done(a) + c;
+        } else if (type == kItemMid) {
+            const int cb = row0 - 2 * C + k * kMidCols;
+            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, cb, cb, 0, kMidCols);
+            counter = sy_fix_done(a) + c;
         } else {
             const int cb = row0 - C + k * kFixCols;
             bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, cb, cb, 0, kFixCols);
@@ -725,12 +750,12 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
         if (tid == 0) {
             // completion counter of this item's queue and chunk (item[] is stable until the next fetch)
             const int ty = ((volatile int*)sh.item)[0], cc = ((volatile int*)sh.item)[1];
-            int* done = (ty == kItemDiag ? sy_diag_done(a) : ty == kItemFix ? sy_fix_done(a) : sy_far_done(a)) + cc;
+            int* done = (ty == kItemDiag ? sy_diag_done(a) : (ty == kItemFix || ty == kItemMid) ? sy_fix_done(a) : sy_far_done(a)) + cc;
             __threadfence();
             atomicAdd(done, 1);
             if (a.dbg) {
                 const unsigned long long dt = (unsigned long long)(clock64() - t_item);
-                atomicAdd((unsigned long long*)a.dbg + 10 + (ty == kItemFarU ? kItemFarL : ty), dt);   // busy cycles: [11] diag [12] far [13] fix
+                atomicAdd((unsigned long long*)a.dbg + 10 + (ty == kItemFarU ? kItemFarL : ty == kItemMid ? kItemFix : ty), dt);   // busy cycles: [11] diag [12] far [13] fix
                 if (near) atomicAdd((unsigned long long*)a.dbg + 14, dt);                              // [14] near workers
             }
         }
