@@ -316,12 +316,12 @@ def run_ours(args, w):
     achieved_instr = bulk_pairs * FP64_INSTR_PER_PAIR / (bulk_ms * 1e-3) if bulk_ms > 0 else 0.0
     total_timed_ms = sum(v[0] for v in timed.values())
     roofline = {
-        "bound": "alu", "kernel": "k_bulk",
+        "bound": "alu", "kernel": "k_sweep (persistent: the whole sweep in one launch)" if bulk_launches == 1 else "k_bulk",
         "achieved": 2.0 * achieved_instr / 1e12, "peak": 2.0 * peak_instr / 1e12, "unit": "TFLOP/s",
         "frac": achieved_instr / peak_instr, "traffic": read_measured_traffic(),
-        "note": ("FP64 plain-ALU pipe; 27 FP64-pipe instructions per pair evaluation counted as one FMA (2 flop) "
-                 "each; peak = 64 lanes/SM x SMs x max SM clock (derived, DESIGN.md); no FP64 entry in "
-                 "MEASURED_PEAKS.json"),
+        "note": ("FP64 plain-ALU pipe; algorithmic count: 27 FP64-pipe instructions per pair evaluation (SURVEY.md "
+                 "8(d)), one FMA (2 flop) each; the kernel executes 22 per pair; peak = 64 lanes/SM x SMs x max SM "
+                 "clock (derived, DESIGN.md); no FP64 entry in MEASURED_PEAKS.json"),
         "launches_per_sweep": bulk_launches, "avg_launch_ms": bulk_ms / max(1, bulk_launches),
         "pairs_per_launch": bulk_pairs / max(1, bulk_launches),
         "measured_dfma_per_s": measured_dfma, "frac_of_measured_dfma": achieved_instr / measured_dfma,

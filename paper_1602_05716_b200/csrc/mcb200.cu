@@ -82,10 +82,10 @@ struct mc_handle {
     bool overlap = true;
     int engine = 1;          // 1: one persistent kernel per sweep (persist.cuh); 0: kernels per chunk in a graph
     int prows = 4;           // rows per consumer thread of the persistent kernel (chunk = 256 * prows)
-    int pfarcols = 128;      // columns per FAR item of the persistent kernel
+    int pfarcols = 256;      // columns per FAR item of the persistent kernel
     int pmode = 0;           // 1: throughput probe (diagnostic; the sweep's results are meaningless)
     bool pwave = true;       // round the FAR items of a chunk to a multiple of the FAR workers
-    int pnear = 16;          // worker CTAs of the persistent kernel that serve FIX and DIAG items only
+    int pnear = 4;           // worker CTAs of the persistent kernel that serve FIX and DIAG items only
     bool debug = false;      // collect the cycle counters of mc_debug_counters
     int pgrid = 0;           // CTAs of the persistent kernel (0: not yet configured)
     int bulk_rows = 1;       // rows per consumer thread of k_bulk (1 or 2)
