@@ -664,63 +664,107 @@ __global__ void k_check_particles(Params p, const double* d) {
 }
 
 // ------------------------------------------------------------------------------------------
-// a5: from-scratch energy (and the overlap check of mc_init).  Row i sums q_j / r_ij over
-// j > i; columns are cut in 256-wide tiles handed round-robin to gridDim.y slices.
-// part[slice][i] is reduced in fixed order by k_energy_reduce.
+// a5: from-scratch energy (and the overlap check of mc_init): E = l_B sum_{i<j} q_i q_j / r_ij.
+// The upper triangle is cut into units of 1024 rows x 1024 columns (4 column tiles of 256); one CTA
+// per unit, 4 rows per thread, columns staged through shared memory, 12 FP64-pipe instructions per
+// pair.  Units on the diagonal test j > i per pair.  Every CTA reduces its rows in a fixed order and
+// writes one partial; k_energy_reduce adds the partials in index order.
 // ------------------------------------------------------------------------------------------
-constexpr int kEnergySlices = 32;
+constexpr int kERows = 4, kEBlock = 256 * kERows, kETile = 256;
 
-__global__ void __launch_bounds__(256) k_energy(Params p, double* part, int check_overlap) {
-    __shared__ double2 sxy[256], szq[256];
-    __shared__ double sh[256];
+__host__ __device__ inline int energy_units(int Np) {
+    const int nrb = (Np + kEBlock - 1) / kEBlock;
+    int n = 0;
+    for (int rb = 0; rb < nrb; ++rb) n += ((Np - rb * kEBlock) + kEBlock - 1) / kEBlock;
+    return n;
+}
+
+template <bool CHECK>
+__global__ void __launch_bounds__(256, 2) k_energy(Params p, double* part) {
+    __shared__ double2 sxy[kETile], szq[kETile];
+    __shared__ double sh[kETile];
+    __shared__ double red[8];
     const int tid = threadIdx.x;
-    const int rg = blockIdx.x, sl = blockIdx.y;
-    const int i = rg * 256 + tid;
-    const bool live = i < p.Np;
-    double2 xyi = make_double2(0, 0), zqi = make_double2(0, 0);
-    double hi = 0;
-    if (live) { xyi = p.xy[i]; zqi = p.zq[i]; hi = p.hh[i]; }
-    double acc = 0.0;
+    // unit -> (row block rb, column block cb >= rb)
+    int unit = blockIdx.x, rb = 0;
+    for (;;) {
+        const int n = ((p.Np - rb * kEBlock) + kEBlock - 1) / kEBlock;
+        if (unit < n) break;
+        unit -= n;
+        ++rb;
+    }
+    const int cb = rb + unit;
+    double x[kERows], y[kERows], z[kERows], q[kERows], h[kERows], acc[kERows];
     int bad = 0;
-    const int ntile = (p.Np + 255) / 256;
-    for (int ct = rg + sl; ct < ntile; ct += kEnergySlices) {
-        const int j0 = ct * 256;
+#pragma unroll
+    for (int u = 0; u < kERows; ++u) {
+        const int i = rb * kEBlock + u * 256 + tid;
+        const bool live = i < p.Np;
+        const double2 xy = live ? p.xy[i] : make_double2(3.0e9, 0.0);
+        const double2 zq = live ? p.zq[i] : make_double2(0.0, 0.0);
+        x[u] = xy.x; y[u] = xy.y; z[u] = zq.x; q[u] = zq.y;
+        h[u] = live ? p.hh[i] : 0.0;
+        acc[u] = 0.0;
+    }
+    for (int ct = 0; ct < kEBlock / kETile; ++ct) {
+        const int j0 = cb * kEBlock + ct * kETile;
+        if (j0 >= p.Np) break;
+        const int cnt = min(kETile, p.Np - j0);
         __syncthreads();
-        if (j0 + tid < p.Np) { sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; sh[tid] = p.hh[j0 + tid]; }
+        if (tid < cnt) { sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; if (CHECK) sh[tid] = p.hh[j0 + tid]; }
         __syncthreads();
-        const int cnt = min(256, p.Np - j0);
-        if (!live) continue;
-#pragma unroll 4
-        for (int j = 0; j < cnt; ++j) {
-            if (j0 + j <= i) continue;
-            const double2 a = sxy[j], b = szq[j];
-            const double r2 = dist2(__dadd_rn(xyi.x, -a.x), __dadd_rn(xyi.y, -a.y), __dadd_rn(zqi.x, -b.x));
-            acc = __fma_rn(b.y, rsqrt_fast(r2), acc);
-            if (check_overlap) {
-                const double sij = __dadd_rn(hi, sh[j]);
-                bad |= (r2 < __dmul_rn(sij, sij)) && (j0 + j < p.N) && (i < p.N);
+        const bool diagonal = cb == rb;
+        if (!diagonal && !CHECK) {
+#pragma unroll 2
+            for (int j = 0; j < cnt; ++j) {
+                const double2 a = sxy[j], b = szq[j];
+#pragma unroll
+                for (int u = 0; u < kERows; ++u) {
+                    const double r2 = dist2(__dadd_rn(x[u], -a.x), __dadd_rn(y[u], -a.y), __dadd_rn(z[u], -b.x));
+                    acc[u] = __fma_rn(b.y, rsqrt_fast(r2), acc[u]);
+                }
+            }
+        } else {
+            for (int j = 0; j < cnt; ++j) {
+                const double2 a = sxy[j], b = szq[j];
+#pragma unroll
+                for (int u = 0; u < kERows; ++u) {
+                    const int i = rb * kEBlock + u * 256 + tid;
+                    if (j0 + j > i) {
+                        const double r2 = dist2(__dadd_rn(x[u], -a.x), __dadd_rn(y[u], -a.y), __dadd_rn(z[u], -b.x));
+                        acc[u] = __fma_rn(b.y, rsqrt_fast(r2), acc[u]);
+                        if (CHECK) {
+                            const double sij = __dadd_rn(h[u], sh[j]);
+                            bad |= (r2 < __dmul_rn(sij, sij)) && (j0 + j < p.N) && (i < p.N);
+                        }
+                    }
+                }
             }
         }
     }
-    if (live) part[(size_t)sl * p.Np + i] = __dmul_rn(zqi.y, acc);
+    // fixed-order reduction: rows of the thread, lanes of the warp, warps of the CTA
+    double v = 0.0;
+#pragma unroll
+    for (int u = 0; u < kERows; ++u) v = __dadd_rn(v, __dmul_rn(q[u], acc[u]));
+    v = warp_sum(v);
+    if ((tid & 31) == 0) red[tid >> 5] = v;
+    __syncthreads();
+    if (tid == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t = __dadd_rn(t, red[w]);
+        part[blockIdx.x] = t;
+    }
     if (bad) atomicMin(&p.st->err, -2);
 }
 
-// out = l_B * sum_i sum_slices part; optionally stored into E_run.  One CTA of 1024 threads.
-__global__ void __launch_bounds__(1024) k_energy_reduce(Params p, const double* part, double* out,
-                                                        int set_running) {
-    __shared__ double red[1024];
+// out = l_B * sum of the partials in index order (one warp; lane l adds partials l, l+32, ...)
+__global__ void __launch_bounds__(32) k_energy_reduce(Params p, const double* part, int nparts, double* out,
+                                                      int set_running) {
     double acc = 0.0;
-    for (int i = threadIdx.x; i < p.Np; i += 1024)
-        for (int sl = 0; sl < kEnergySlices; ++sl) acc += part[(size_t)sl * p.Np + i];
-    red[threadIdx.x] = acc;
-    __syncthreads();
-    for (int o = 512; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
-        __syncthreads();
-    }
+    for (int k = threadIdx.x; k < nparts; k += 32) acc = __dadd_rn(acc, part[k]);
+    acc = warp_sum(acc);
     if (threadIdx.x == 0) {
-        const double E = __dmul_rn(p.lB, red[0]);
+        const double E = __dmul_rn(p.lB, acc);
         if (out) *out = E;
         if (set_running) p.st->E_run = E;
     }
@@ -775,12 +819,140 @@ __global__ void __launch_bounds__(1024) k_centres(Params p, double centre_rmax, 
     }
 }
 
-constexpr int kHistSlices = 16;
+constexpr int kHistSlices = 8;
+constexpr int kCellBits = 5, kCellDim = 1 << kCellBits, kCells = 1 << (3 * kCellBits);
 
-__global__ void __launch_bounds__(256) k_hist(Params p, const int* list, const int* count, double inv_w,
-                                              int nbins, double cut2, unsigned long long* hist) {
+// The partners of a centre within nbins * bin_width are found through a spatially sorted copy of
+// the configuration: particles are counting-sorted by the Morton code of their cell (k_cell_*), so
+// that 256 consecutive particles fill a compact box; k_hist takes 256 consecutive centres and skips
+// every 256-particle column tile whose bounding box is farther than the histogram's range from the
+// centres' bounding box.  The counts do not depend on the order inside a cell (integer adds).
+struct CellGrid {
+    double lo, inv_edge;   // cell coordinate = clamp(floor((x - lo) * inv_edge), 0, dim - 1)
+    int dim;
+};
+__device__ __forceinline__ unsigned spread5(unsigned v) {   // abcde -> a00b00c00d00e
+    return (v & 1u) | ((v & 2u) << 2) | ((v & 4u) << 4) | ((v & 8u) << 6) | ((v & 16u) << 8);
+}
+__device__ __forceinline__ int cell_code(const CellGrid& g, double x, double y, double z) {
+    const int cx = min(g.dim - 1, max(0, (int)floor((x - g.lo) * g.inv_edge)));
+    const int cy = min(g.dim - 1, max(0, (int)floor((y - g.lo) * g.inv_edge)));
+    const int cz = min(g.dim - 1, max(0, (int)floor((z - g.lo) * g.inv_edge)));
+    return (int)(spread5((unsigned)cx) | (spread5((unsigned)cy) << 1) | (spread5((unsigned)cz) << 2));
+}
+__global__ void __launch_bounds__(256) k_cell_count(Params p, CellGrid g, int* code, int* count) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.N) return;
+    const double2 xy = p.xy[i];
+    const int c = cell_code(g, xy.x, xy.y, p.zq[i].x);
+    code[i] = c;
+    atomicAdd(count + c, 1);
+}
+// exclusive scan of count[kCells] into cursor[kCells]; one CTA of 1024 threads, 32 cells each
+__global__ void __launch_bounds__(1024) k_cell_scan(const int* count, int* cursor) {
+    __shared__ int wsum[32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int per = kCells / 1024;
+    int loc[per], tot = 0;
+#pragma unroll
+    for (int k = 0; k < per; ++k) { loc[k] = tot; tot += count[tid * per + k]; }
+    int inc = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        int w = wsum[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, w, o);
+            if (lane >= o) w += v;
+        }
+        wsum[lane] = w;
+    }
+    __syncthreads();
+    const int base = inc - tot + (warp > 0 ? wsum[warp - 1] : 0);
+#pragma unroll
+    for (int k = 0; k < per; ++k) cursor[tid * per + k] = base + loc[k];
+}
+__global__ void __launch_bounds__(256) k_cell_fill(Params p, const int* code, int* cursor, double2* sxy, double2* szq) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.N) return;
+    const int pos = atomicAdd(cursor + code[i], 1);
+    sxy[pos] = p.xy[i];
+    szq[pos] = p.zq[i];
+}
+// bounding box of every tile of 256 consecutive sorted particles: bbox[t] = {xmin, xmax, ymin, ymax, zmin, zmax}
+__global__ void __launch_bounds__(256) k_tile_bbox(const double2* sxy, const double2* szq, int N, double* bbox) {
+    __shared__ double red[8][6];
+    const int tid = threadIdx.x, j = blockIdx.x * 256 + tid;
+    double v[6] = {1e300, -1e300, 1e300, -1e300, 1e300, -1e300};
+    if (j < N) {
+        const double2 a = sxy[j];
+        const double z = szq[j].x;
+        v[0] = v[1] = a.x; v[2] = v[3] = a.y; v[4] = v[5] = z;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const double w = __shfl_xor_sync(0xffffffffu, v[k], o);
+            v[k] = (k & 1) ? fmax(v[k], w) : fmin(v[k], w);
+        }
+    if ((tid & 31) == 0)
+        for (int k = 0; k < 6; ++k) red[tid >> 5][k] = v[k];
+    __syncthreads();
+    if (tid < 6) {
+        double r = red[0][tid];
+        for (int w = 1; w < 8; ++w) r = (tid & 1) ? fmax(r, red[w][tid]) : fmin(r, red[w][tid]);
+        bbox[blockIdx.x * 6 + tid] = r;
+    }
+}
+
+// centres (|x_i| <= centre_rmax) of the sorted copy, compacted per 1024-particle block (blocks land
+// in the list in completion order, each block's centres stay together and in order)
+__global__ void __launch_bounds__(1024) k_centres_sorted(Params p, double centre_rmax, int* list, int* count,
+                                                         unsigned long long* n_centres) {
+    __shared__ int wcount[32];
+    __shared__ int base;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int i = blockIdx.x * 1024 + tid;
+    const double c2 = __dmul_rn(centre_rmax, centre_rmax);
+    bool is = false;
+    int sp = 0;
+    if (i < p.N) {
+        const double2 xy = p.xy[i];
+        const double2 zq = p.zq[i];
+        is = dist2(xy.x, xy.y, zq.x) <= c2;
+        sp = zq.y > 0.0 ? 0 : 1;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, is);
+    const unsigned m0 = __ballot_sync(0xffffffffu, is && sp == 0);
+    if (lane == 0) {
+        wcount[warp] = __popc(m);
+        if (m0) atomicAdd(n_centres + 0, (unsigned long long)__popc(m0));
+        if (m & ~m0) atomicAdd(n_centres + 1, (unsigned long long)__popc(m & ~m0));
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int tot = 0;
+        for (int w = 0; w < 32; ++w) { const int c = wcount[w]; wcount[w] = tot; tot += c; }
+        base = tot ? atomicAdd(count, tot) : 0;
+    }
+    __syncthreads();
+    if (is) list[base + wcount[warp] + __popc(m & ((1u << lane) - 1u))] = i;
+}
+
+// p.xy / p.zq here are the SORTED copies; list = sorted indices of the centres
+__global__ void __launch_bounds__(256) k_hist(Params p, const int* list, const int* count, const double* bbox,
+                                              double inv_w, int nbins, double cut2, unsigned long long* hist) {
     extern __shared__ unsigned shist[];  // [4][nbins]
     __shared__ double2 sxy[256], szq[256];
+    __shared__ double cred[8][6];
+    __shared__ double cbox[6];
     const int tid = threadIdx.x;
     const int nc = *count;
     if ((int)blockIdx.x * 256 >= nc) return;
@@ -791,8 +963,38 @@ __global__ void __launch_bounds__(256) k_hist(Params p, const int* list, const i
     double2 xyi = make_double2(0, 0), zqi = make_double2(0, 0);
     if (live) { xyi = p.xy[i]; zqi = p.zq[i]; }
     const int si = zqi.y > 0.0 ? 0 : 1;
+    // bounding box of this block's centres
+    {
+        double v[6] = {1e300, -1e300, 1e300, -1e300, 1e300, -1e300};
+        if (live) { v[0] = v[1] = xyi.x; v[2] = v[3] = xyi.y; v[4] = v[5] = zqi.x; }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+            for (int k = 0; k < 6; ++k) {
+                const double w = __shfl_xor_sync(0xffffffffu, v[k], o);
+                v[k] = (k & 1) ? fmax(v[k], w) : fmin(v[k], w);
+            }
+        if ((tid & 31) == 0)
+            for (int k = 0; k < 6; ++k) cred[tid >> 5][k] = v[k];
+        __syncthreads();
+        if (tid < 6) {
+            double r = cred[0][tid];
+            for (int w = 1; w < 8; ++w) r = (tid & 1) ? fmax(r, cred[w][tid]) : fmin(r, cred[w][tid]);
+            cbox[tid] = r;
+        }
+        __syncthreads();
+    }
     const int ntile = (p.N + 255) / 256;
+    const double margin = 1.0 + 1e-6;   // the cull is conservative: only tiles clearly out of range are skipped
     for (int ct = blockIdx.y; ct < ntile; ct += kHistSlices) {
+        // squared distance between the two boxes
+        double d2 = 0.0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double gap = fmax(0.0, fmax(bbox[ct * 6 + 2 * k] - cbox[2 * k + 1], cbox[2 * k] - bbox[ct * 6 + 2 * k + 1]));
+            d2 += gap * gap;
+        }
+        if (d2 > cut2 * margin) continue;   // same decision in every thread
         const int j0 = ct * 256;
         __syncthreads();
         if (j0 + tid < p.N) { sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; }

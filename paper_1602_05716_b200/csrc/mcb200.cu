@@ -34,7 +34,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t xy, zq, hh, lbq, txy, tz, lnu, wall, partA, ovA, partD, ovD, Dblk, OVold, OVnew, log_dE, log_flags,
-        st, epart, centres, ccount, stage_pos, S1, S2, ovc, sy, dbg, total;
+        st, epart, centres, ccount, stage_pos, S1, S2, ovc, sy, dbg, hcode, hcount, hcursor, hsxy, hszq, hbbox, total;
 };
 
 int padded(int64_t N) { return (int)((N + kTile - 1) / kTile * kTile); }
@@ -57,9 +57,11 @@ Layout make_layout(int64_t N) {
     L.sy = take((size_t)(kSyHdr + 4 * (Np / 256 + 1)) * 4);
     take(65536);
     L.dbg = take(16 * 8 + 1024 * 8);
+    L.hcode = take(Np * 4); L.hcount = take((size_t)kCells * 4); L.hcursor = take((size_t)kCells * 4);
+    L.hsxy = take(Np * 16); L.hszq = take(Np * 16); L.hbbox = take((Np / 256 + 1) * 6 * 8);
     L.log_dE = take(Np * 8); L.log_flags = take(Np);
     L.st = take(sizeof(DevState));
-    L.epart = take((size_t)kEnergySlices * Np * 8 + 8);
+    L.epart = take(((size_t)energy_units((int)Np) + 2) * 8);
     L.centres = take(Np * 4); L.ccount = take(16);
     L.stage_pos = take(3 * (size_t)N * 8);
     L.total = off;
@@ -308,9 +310,10 @@ int build_graph(mc_handle* h) {
 
 int enqueue_energy(mc_handle* h, double* out_dev, int set_running, int check_overlap) {
     const Params& p = h->p;
-    dim3 grid((p.Np + 255) / 256, kEnergySlices);
-    k_energy<<<grid, 256, 0, h->stream>>>(p, h->epart, check_overlap);
-    k_energy_reduce<<<1, 1024, 0, h->stream>>>(p, h->epart, out_dev, set_running);
+    const int units = energy_units(p.Np);
+    if (check_overlap) k_energy<true><<<units, 256, 0, h->stream>>>(p, h->epart);
+    else k_energy<false><<<units, 256, 0, h->stream>>>(p, h->epart);
+    k_energy_reduce<<<1, 32, 0, h->stream>>>(p, h->epart, units, out_dev, set_running);
     h->launches += 2;
     CUDA_TRY(cudaGetLastError());
     return MC_OK;
@@ -445,7 +448,7 @@ int mc_sweep(mc_handle* h, int64_t n) {
 
 int mc_energy(mc_handle* h, double* E_host) {
     if (!h || !E_host) return fail(MC_EINVAL, "null argument");
-    double* out = h->epart + (size_t)kEnergySlices * h->p.Np;
+    double* out = h->epart + (size_t)energy_units(h->p.Np);
     const int rc = enqueue_energy(h, out, 0, 0);
     if (rc != MC_OK) return rc;
     CUDA_TRY(cudaMemcpyAsync(E_host, out, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
@@ -519,15 +522,37 @@ int mc_pair_hist(mc_handle* h, double bin_width, int nbins, double centre_rmax, 
     const double inv_w = 1.0 / bin_width;
     const double rcut = (double)nbins * bin_width * (1.0 + 1e-9);
     const double cut2 = rcut * rcut;
-    k_centres<<<1, 1024, 0, h->stream>>>(p, centre_rmax, h->centres, h->ccount,
-                                         (unsigned long long*)n_centres_dev);
+    // spatially sorted copy of the configuration (Morton order of cells of about rcut / 2)
+    CellGrid g{};
+    g.dim = (int)std::min<double>(kCellDim, std::max(1.0, std::floor(2.0 * p.R / (0.5 * rcut))));
+    g.lo = -p.R;
+    g.inv_edge = (double)g.dim / (2.0 * p.R);
+    char* w = h->ws;
+    int* code = (int*)(w + h->L.hcode);
+    int* ccnt = (int*)(w + h->L.hcount);
+    int* ccur = (int*)(w + h->L.hcursor);
+    double2* sxy = (double2*)(w + h->L.hsxy);
+    double2* szq = (double2*)(w + h->L.hszq);
+    double* bbox = (double*)(w + h->L.hbbox);
+    const int nb = (p.N + 255) / 256;
+    CUDA_TRY(cudaMemsetAsync(ccnt, 0, (size_t)kCells * 4, h->stream));
+    CUDA_TRY(cudaMemsetAsync(h->ccount, 0, 4, h->stream));
+    k_cell_count<<<nb, 256, 0, h->stream>>>(p, g, code, ccnt);
+    k_cell_scan<<<1, 1024, 0, h->stream>>>(ccnt, ccur);
+    k_cell_fill<<<nb, 256, 0, h->stream>>>(p, code, ccur, sxy, szq);
+    k_tile_bbox<<<nb, 256, 0, h->stream>>>(sxy, szq, p.N, bbox);
+    Params ps = p;
+    ps.xy = sxy;
+    ps.zq = szq;
+    k_centres_sorted<<<(p.N + 1023) / 1024, 1024, 0, h->stream>>>(ps, centre_rmax, h->centres, h->ccount,
+                                                                 (unsigned long long*)n_centres_dev);
     const size_t smem = (size_t)4 * nbins * sizeof(unsigned);
-    if (smem > 40 * 1024)
+    if (smem > 32 * 1024)
         CUDA_TRY(cudaFuncSetAttribute(k_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    dim3 grid((p.N + 255) / 256, kHistSlices);
-    k_hist<<<grid, 256, smem, h->stream>>>(p, h->centres, h->ccount, inv_w, nbins, cut2,
+    dim3 grid(nb, kHistSlices);
+    k_hist<<<grid, 256, smem, h->stream>>>(ps, h->centres, h->ccount, bbox, inv_w, nbins, cut2,
                                            (unsigned long long*)hist_dev);
-    h->launches += 2;
+    h->launches += 6;
     CUDA_TRY(cudaGetLastError());
     return MC_OK;
 }
