@@ -819,8 +819,8 @@ __global__ void __launch_bounds__(1024) k_centres(Params p, double centre_rmax, 
     }
 }
 
-constexpr int kHistSlices = 8;
-constexpr int kCellBits = 5, kCellDim = 1 << kCellBits, kCells = 1 << (3 * kCellBits);
+constexpr int kHistSlices = 32;
+constexpr int kCellBits = 4, kCellDim = 1 << kCellBits, kCells = 1 << (3 * kCellBits);
 
 // The partners of a centre within nbins * bin_width are found through a spatially sorted copy of
 // the configuration: particles are counting-sorted by the Morton code of their cell (k_cell_*), so
@@ -831,8 +831,8 @@ struct CellGrid {
     double lo, inv_edge;   // cell coordinate = clamp(floor((x - lo) * inv_edge), 0, dim - 1)
     int dim;
 };
-__device__ __forceinline__ unsigned spread5(unsigned v) {   // abcde -> a00b00c00d00e
-    return (v & 1u) | ((v & 2u) << 2) | ((v & 4u) << 4) | ((v & 8u) << 6) | ((v & 16u) << 8);
+__device__ __forceinline__ unsigned spread5(unsigned v) {   // dcba -> d00c00b00a
+    return (v & 1u) | ((v & 2u) << 2) | ((v & 4u) << 4) | ((v & 8u) << 6);
 }
 __device__ __forceinline__ int cell_code(const CellGrid& g, double x, double y, double z) {
     const int cx = min(g.dim - 1, max(0, (int)floor((x - g.lo) * g.inv_edge)));
@@ -885,9 +885,9 @@ __global__ void __launch_bounds__(256) k_cell_fill(Params p, const int* code, in
     sxy[pos] = p.xy[i];
     szq[pos] = p.zq[i];
 }
-// bounding box of every tile of 256 consecutive sorted particles: bbox[t] = {xmin, xmax, ymin, ymax, zmin, zmax}
+// bounding box of every sub-tile of 64 consecutive sorted particles: bbox[t] = {xmin, xmax, ymin, ymax, zmin, zmax}
+constexpr int kSubTile = 64;
 __global__ void __launch_bounds__(256) k_tile_bbox(const double2* sxy, const double2* szq, int N, double* bbox) {
-    __shared__ double red[8][6];
     const int tid = threadIdx.x, j = blockIdx.x * 256 + tid;
     double v[6] = {1e300, -1e300, 1e300, -1e300, 1e300, -1e300};
     if (j < N) {
@@ -902,13 +902,14 @@ __global__ void __launch_bounds__(256) k_tile_bbox(const double2* sxy, const dou
             const double w = __shfl_xor_sync(0xffffffffu, v[k], o);
             v[k] = (k & 1) ? fmax(v[k], w) : fmin(v[k], w);
         }
+    __shared__ double red[8][6];
     if ((tid & 31) == 0)
         for (int k = 0; k < 6; ++k) red[tid >> 5][k] = v[k];
     __syncthreads();
-    if (tid < 6) {
-        double r = red[0][tid];
-        for (int w = 1; w < 8; ++w) r = (tid & 1) ? fmax(r, red[w][tid]) : fmin(r, red[w][tid]);
-        bbox[blockIdx.x * 6 + tid] = r;
+    if (tid < 24) {   // 4 sub-tiles x 6 values, each from 2 warps
+        const int st = tid / 6, k = tid % 6;
+        const double a = red[2 * st][k], b = red[2 * st + 1][k];
+        bbox[((size_t)blockIdx.x * 4 + st) * 6 + k] = (k & 1) ? fmax(a, b) : fmin(a, b);
     }
 }
 
@@ -986,30 +987,40 @@ __global__ void __launch_bounds__(256) k_hist(Params p, const int* list, const i
     }
     const int ntile = (p.N + 255) / 256;
     const double margin = 1.0 + 1e-6;   // the cull is conservative: only tiles clearly out of range are skipped
-    for (int ct = blockIdx.y; ct < ntile; ct += kHistSlices) {
-        // squared distance between the two boxes
-        double d2 = 0.0;
+    for (int ct = blockIdx.y; ct < ntile; ct += gridDim.y) {
+        // which of the tile's 4 sub-tiles of 64 are in range of this block's centres (same in every thread)
+        unsigned inrange = 0u;
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const double gap = fmax(0.0, fmax(bbox[ct * 6 + 2 * k] - cbox[2 * k + 1], cbox[2 * k] - bbox[ct * 6 + 2 * k + 1]));
-            d2 += gap * gap;
+        for (int st = 0; st < 4; ++st) {
+            const double* bb = bbox + ((size_t)ct * 4 + st) * 6;
+            double d2 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double gap = fmax(0.0, fmax(bb[2 * k] - cbox[2 * k + 1], cbox[2 * k] - bb[2 * k + 1]));
+                d2 += gap * gap;
+            }
+            if (d2 <= cut2 * margin) inrange |= 1u << st;
         }
-        if (d2 > cut2 * margin) continue;   // same decision in every thread
+        if (inrange == 0u) continue;
         const int j0 = ct * 256;
         __syncthreads();
         if (j0 + tid < p.N) { sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; }
         __syncthreads();
         const int cnt = min(256, p.N - j0);
         if (!live) continue;
+        for (int st = 0; st < 4; ++st) {
+            if (!((inrange >> st) & 1u)) continue;
+            const int jend = min(cnt, (st + 1) * kSubTile);
 #pragma unroll 4
-        for (int j = 0; j < cnt; ++j) {
-            const double2 a = sxy[j], b = szq[j];
-            const double r2 = dist2(__dadd_rn(xyi.x, -a.x), __dadd_rn(xyi.y, -a.y), __dadd_rn(zqi.x, -b.x));
-            if (r2 < cut2 && (j0 + j) != i) {
-                const double fb = floor(__dmul_rn(sqrt(r2), inv_w));
-                if (fb < (double)nbins) {
-                    const int sj = b.y > 0.0 ? 0 : 1;
-                    atomicAdd(&shist[(si * 2 + sj) * nbins + (int)fb], 1u);
+            for (int j = st * kSubTile; j < jend; ++j) {
+                const double2 a = sxy[j], b = szq[j];
+                const double r2 = dist2(__dadd_rn(xyi.x, -a.x), __dadd_rn(xyi.y, -a.y), __dadd_rn(zqi.x, -b.x));
+                if (r2 < cut2 && (j0 + j) != i) {
+                    const double fb = floor(__dmul_rn(sqrt(r2), inv_w));
+                    if (fb < (double)nbins) {
+                        const int sj = b.y > 0.0 ? 0 : 1;
+                        atomicAdd(&shist[(si * 2 + sj) * nbins + (int)fb], 1u);
+                    }
                 }
             }
         }

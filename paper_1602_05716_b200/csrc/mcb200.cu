@@ -58,7 +58,7 @@ Layout make_layout(int64_t N) {
     take(65536);
     L.dbg = take(16 * 8 + 1024 * 8);
     L.hcode = take(Np * 4); L.hcount = take((size_t)kCells * 4); L.hcursor = take((size_t)kCells * 4);
-    L.hsxy = take(Np * 16); L.hszq = take(Np * 16); L.hbbox = take((Np / 256 + 1) * 6 * 8);
+    L.hsxy = take(Np * 16); L.hszq = take(Np * 16); L.hbbox = take((Np / 256 + 1) * 4 * 6 * 8);
     L.log_dE = take(Np * 8); L.log_flags = take(Np);
     L.st = take(sizeof(DevState));
     L.epart = take(((size_t)energy_units((int)Np) + 2) * 8);
@@ -85,6 +85,7 @@ struct mc_handle {
     int engine = 1;          // 1: one persistent kernel per sweep (persist.cuh); 0: kernels per chunk in a graph
     int prows = 4;           // rows per consumer thread of the persistent kernel (chunk = 256 * prows)
     int pfarcols = 256;      // columns per FAR item of the persistent kernel
+    int hist_slices = kHistSlices;   // column slices (grid.y) of k_hist
     int pmode = 0;           // 1: throughput probe (diagnostic; the sweep's results are meaningless)
     bool pwave = true;       // round the FAR items of a chunk to a multiple of the FAR workers
     int pnear = 4;           // worker CTAs of the persistent kernel that serve FIX and DIAG items only
@@ -549,7 +550,7 @@ int mc_pair_hist(mc_handle* h, double bin_width, int nbins, double centre_rmax, 
     const size_t smem = (size_t)4 * nbins * sizeof(unsigned);
     if (smem > 32 * 1024)
         CUDA_TRY(cudaFuncSetAttribute(k_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    dim3 grid(nb, kHistSlices);
+    dim3 grid(nb, h->hist_slices);
     k_hist<<<grid, 256, smem, h->stream>>>(ps, h->centres, h->ccount, bbox, inv_w, nbins, cut2,
                                            (unsigned long long*)hist_dev);
     h->launches += 6;
@@ -673,6 +674,9 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     } else if (!std::strcmp(key, "far_cols")) {
         if (value < 8 || value > 65536 || value % 8) return fail(MC_EINVAL, "far_cols must be a multiple of 8 in 8..65536");
         h->pfarcols = (int)value;
+    } else if (!std::strcmp(key, "hist_slices")) {
+        if (value < 1 || value > 64) return fail(MC_EINVAL, "hist_slices must be in 1..64");
+        h->hist_slices = (int)value;
     } else if (!std::strcmp(key, "probe")) {
         h->pmode = value != 0 ? 1 : 0;
     } else if (!std::strcmp(key, "wave")) {

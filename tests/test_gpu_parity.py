@@ -209,8 +209,13 @@ def test_strong_coupling_low_acceptance():
 # ---------------------------------------------------------------------------------------------------
 # host logic of the library: options, re-entrancy, resume, validation
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("opts", [{"chunk": 32}, {"chunk": 96}, {"chunk": 512}, {"graph": 0}, {"overlap": 0},
-                                  {"graph": 0, "chunk": 256}])
+@pytest.mark.parametrize("opts", [
+    # persistent engine (the default): rows per thread / chunk size, item width, near workers, wave rounding
+    {"prows": 1}, {"prows": 2}, {"prows": 4}, {"far_cols": 64}, {"far_cols": 1024}, {"pnear": 0}, {"pnear": 32},
+    {"wave": 0}, {"prows": 2, "far_cols": 8, "pnear": 1}, {"debug": 1},
+    # kernels-per-chunk engine
+    {"engine": 0}, {"engine": 0, "chunk": 32}, {"engine": 0, "chunk": 96}, {"engine": 0, "chunk": 512},
+    {"engine": 0, "graph": 0}, {"engine": 0, "overlap": 0}, {"engine": 0, "graph": 0, "chunk": 256}])
 def test_every_launch_configuration_gives_the_same_chain(opts):
     w = W.scaled(W.CONFIGS[2], 2500)
     g, o = make_pair(w)
@@ -218,6 +223,39 @@ def test_every_launch_configuration_gives_the_same_chain(opts):
         g.mc_set_option(k, v)
     r = lockstep(g, o, 4, tag=str(opts))
     assert_stats_equal(g, o, r["near_tie_flips"])
+
+
+@pytest.mark.parametrize("N,prows", [(700, 1), (5000, 2), (5000, 4), (20000, 4)])
+def test_persistent_kernel_is_bit_reproducible(N, prows):
+    """Which CTA runs which item, and in what order, differs from run to run; the fixed-point accumulation
+    makes every sum -- and so the whole trial log -- independent of it."""
+    from paper_1602_05716_b200.binding import MCSystem
+    w = W.scaled(W.CONFIGS[3], N)
+    pos, q, d = w.arrays()
+    logs = []
+    for rep in range(3):
+        g = MCSystem(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 5)
+        g.mc_set_option("prows", prows)
+        g.mc_set_option("pnear", (0, 4, 16)[rep])     # perturbs the schedule, not the items
+        g.mc_sweep(6)
+        lg = g.mc_get_trial_log()
+        logs.append((g.positions.copy(), lg["dE"].copy(), lg["flags"].copy(), g.mc_get_stats()))
+    for other in logs[1:]:
+        assert np.array_equal(logs[0][0], other[0])
+        assert np.array_equal(logs[0][1], other[1], equal_nan=True)
+        assert np.array_equal(logs[0][2], other[2])
+        assert logs[0][3] == other[3]
+
+
+def test_many_sweeps_never_stall():
+    """200 sweeps of a mid-size system: the watchdog (MC_ESTALL) must stay silent and the invariants hold."""
+    w = W.scaled(W.CONFIGS[1], 6000)
+    g, o = make_pair(w)
+    g.mc_sweep(200)
+    st = g.mc_get_stats()                      # raises on MC_ESTALL
+    assert hard_constraints_ok(g.positions, w.arrays()[2], w.cavity_R)
+    e = g.mc_energy()
+    assert abs(st["E_running"] - e) < 1e-8 * max(1.0, abs(e))
 
 
 def test_reentrancy_and_resume():
