@@ -34,6 +34,7 @@ struct Params {
     unsigned long long seed;
     int* sy; int sy_n;         // scheduling state of the persistent sweep kernel (zeroed by k_trial)
     long long* S1; long long* S2; int* ovc;   // [Np] per-row fixed-point sums / overlap counts (persistent kernel)
+    double* nn;                // [Np] |x_i|^2 of the current positions (persistent kernel's distance form)
 };
 
 // Order-independent accumulation of a row's partial sums (persistent kernel): the double is split
@@ -101,6 +102,7 @@ struct __align__(16) ColStage {
     double2 xy[kColTile];
     double2 zq[kColTile];
     double h[kColTile];
+    double n[kColTile];
 };
 
 // slice boundaries in the virtual column space: multiples of 8, so that every staged segment
@@ -542,6 +544,7 @@ k_chain(Params p, int row0, int nrows, int nslots, int last_chunk) {
                 const double q = p.zq[i].y;
                 p.xy[i] = txy;
                 p.zq[i] = make_double2(tz, q);
+                p.nn[i] = dist2(txy.x, txy.y, tz);
             }
             p.log_dE[i] = dE;
             p.log_flags[i] = (unsigned char)((acc ? kFlagAccept : 0u) | (ovv ? kFlagOverlap : 0u) |
@@ -611,6 +614,7 @@ __global__ void k_pack(Params p, const double* pos, const double* q, const doubl
     if (i >= p.Np) return;
     if (i < p.N) {
         p.xy[i] = make_double2(pos[i], pos[(size_t)p.N + i]);
+        p.nn[i] = dist2(pos[i], pos[(size_t)p.N + i], pos[2 * (size_t)p.N + i]);
         if (q) {
             p.zq[i] = make_double2(pos[2 * (size_t)p.N + i], q[i]);
             p.hh[i] = __dmul_rn(0.5, d[i]);
@@ -620,6 +624,7 @@ __global__ void k_pack(Params p, const double* pos, const double* q, const doubl
         }
     } else if (q) {
         p.xy[i] = make_double2(kGhostCoord + kGhostStep * (double)(i - p.N), 0.0);
+        p.nn[i] = __dmul_rn(kGhostCoord + kGhostStep * (double)(i - p.N), kGhostCoord + kGhostStep * (double)(i - p.N));
         p.zq[i] = make_double2(0.0, 0.0);
         p.hh[i] = 0.0;
         p.lbq[i] = 0.0;

@@ -34,7 +34,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t xy, zq, hh, lbq, txy, tz, lnu, wall, partA, ovA, partD, ovD, Dblk, OVold, OVnew, log_dE, log_flags,
-        st, epart, centres, ccount, stage_pos, S1, S2, ovc, sy, dbg, hcode, hcount, hcursor, hsxy, hszq, hbbox, total;
+        st, epart, centres, ccount, stage_pos, S1, S2, ovc, nn, sy, dbg, hcode, hcount, hcursor, hsxy, hszq, hbbox, total;
 };
 
 int padded(int64_t N) { return (int)((N + kTile - 1) / kTile * kTile); }
@@ -52,7 +52,7 @@ Layout make_layout(int64_t N) {
     L.partD = take(2 * nt * kChunkMax * 8); L.ovD = take(2 * nt * kChunkMax * 4);
     L.Dblk = take(2 * (nt * (nt + 1) / 2) * kTile * kTile * 8);
     L.OVold = take((size_t)2 * kChunkMax * nt * 4); L.OVnew = take((size_t)2 * kChunkMax * nt * 4);
-    L.S1 = take(Np * 8); L.S2 = take(Np * 8); L.ovc = take(Np * 4);
+    L.S1 = take(Np * 8); L.S2 = take(Np * 8); L.ovc = take(Np * 4); L.nn = take(Np * 8);
     take(65536);
     L.sy = take((size_t)(kSyHdr + 4 * (Np / 256 + 1)) * 4);
     take(65536);
@@ -369,6 +369,7 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     p.log_dE = (double*)(w + L.log_dE); p.log_flags = (unsigned char*)(w + L.log_flags);
     p.st = (DevState*)(w + L.st);
     p.sy = (int*)(w + L.sy);
+    p.nn = (double*)(w + L.nn);
     p.S1 = (long long*)(w + L.S1); p.S2 = (long long*)(w + L.S2); p.ovc = (int*)(w + L.ovc);
     p.sy_n = kSyHdr + 4 * (p.Np / 256 + 1);   // header + per-chunk counters
     h->prows = p.Np >= 16384 ? 4 : (p.Np >= 2048 ? 2 : 1);

@@ -190,6 +190,37 @@ __device__ __noinline__ int recheck_overlap_cg(const double2* xy, const double2*
     return ov;
 }
 
+// Pair evaluation of the persistent kernel: 20 FP64-pipe instructions (22 if diameters differ) + 2 MUFU.
+//   r2o = |x_i|^2 + |x_j|^2 - 2 x_i.x_j           1 DADD + 3 DFMA   (n_j = |x_j|^2 is staged with the column)
+//   w   = 2 D.x_i + |D|^2 - 2 D.x_j               3 DFMA            (D = x~_i - x_i)
+//   r2n = r2o + w                                 1 DADD
+// The Gram form of r2o carries an absolute error of a few ulp of |x|^2 (<= 3e-13 for |x| <= 34 sigma):
+// far below the 2^-16 band inside which the veto is re-examined exactly, and 1e-13 relative in 1/r at contact.
+struct RowG {
+    double mx, my, mz;  // -2 x_i
+    double n;           // |x_i|^2
+    double ex, ey, ez;  // -2 D
+    double cp;          // 2 D.x_i + |D|^2
+    double h;           // d/2
+    double acc;
+    int m;              // running minimum of the overlap key
+};
+
+template <bool UNIFORM>
+__device__ __forceinline__ int pair_eval_g(RowG& r, const double2 a, const double2 b, double nj, double hj) {
+    const double r2o = __fma_rn(r.mx, a.x, __fma_rn(r.my, a.y, __fma_rn(r.mz, b.x, __dadd_rn(r.n, nj))));
+    const double w = __fma_rn(r.ex, a.x, __fma_rn(r.ey, a.y, __fma_rn(r.ez, b.x, r.cp)));
+    const double r2n = __dadd_rn(r2o, w);
+    int key = __double2hiint(r2n);
+    if (!UNIFORM) {
+        const double sij = __dadd_rn(r.h, hj);
+        key -= __double2hiint(__dmul_rn(sij, sij));
+    }
+    const double du = __dadd_rn(rsqrt_fast(r2n), -rsqrt_fast(r2o));
+    r.acc = __fma_rn(b.y, du, r.acc);
+    return key;
+}
+
 // FAR / FIX item: all rows of the chunk (ROWS per consumer thread) x virtual columns [v0, v1) of
 // the column space that starts at cbeg and skips [gap0, gap1).  Same inner loop as k_bulk; the
 // mbarrier ring persists across items (kring = stages used so far, identical in every thread).
@@ -210,9 +241,10 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
         const int a = cbeg + ((vp < gapv) ? vp : vp + gap);
         const unsigned s = kp % kStages;
         if (kp >= (unsigned)kStages) mbar_wait_wd(wd, &sh.empty_bar[s], ((kp / kStages) - 1) & 1);
-        mbar_arrive_expect_tx(&sh.full_bar[s], (uint32_t)cnt * (UNIFORM ? 32u : 40u));
+        mbar_arrive_expect_tx(&sh.full_bar[s], (uint32_t)cnt * (UNIFORM ? 40u : 48u));
         bulk_g2s(sh.u.w.stage[s].xy, p.xy + a, (uint32_t)cnt * 16u, &sh.full_bar[s]);
         bulk_g2s(sh.u.w.stage[s].zq, p.zq + a, (uint32_t)cnt * 16u, &sh.full_bar[s]);
+        bulk_g2s(sh.u.w.stage[s].n, p.nn + a, (uint32_t)cnt * 8u, &sh.full_bar[s]);
         if (!UNIFORM) bulk_g2s(sh.u.w.stage[s].h, p.hh + a, (uint32_t)cnt * 8u, &sh.full_bar[s]);
         vp += cnt;
         ++kp;
@@ -222,17 +254,20 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
         for (int q = 0; q < kStages - 1 && vp < v1; ++q) issue();
     }
 
-    RowRegs R[ROWS];
+    RowG R[ROWS];
 #pragma unroll
     for (int u = 0; u < ROWS; ++u) {
         const int r = u * kBulkThreads + tid;
         const int i = row0 + (r < nrows ? r : 0);
         const double2 xyi = ldcg2(p.xy + i);
+        const double zi = __ldcg(&p.zq[i].x);
         const double2 txyi = p.txy[i];
-        R[u].x = xyi.x; R[u].y = xyi.y; R[u].z = __ldcg(&p.zq[i].x);
-        const double Dx = __dadd_rn(txyi.x, -xyi.x), Dy = __dadd_rn(txyi.y, -xyi.y), Dz = __dadd_rn(p.tz[i], -R[u].z);
-        R[u].ex = __dadd_rn(Dx, Dx); R[u].ey = __dadd_rn(Dy, Dy); R[u].ez = __dadd_rn(Dz, Dz);
-        R[u].c = dist2(Dx, Dy, Dz);
+        const double Dx = __dadd_rn(txyi.x, -xyi.x), Dy = __dadd_rn(txyi.y, -xyi.y), Dz = __dadd_rn(p.tz[i], -zi);
+        R[u].mx = __dmul_rn(-2.0, xyi.x); R[u].my = __dmul_rn(-2.0, xyi.y); R[u].mz = __dmul_rn(-2.0, zi);
+        R[u].n = __ldcg(p.nn + i);
+        R[u].ex = __dmul_rn(-2.0, Dx); R[u].ey = __dmul_rn(-2.0, Dy); R[u].ez = __dmul_rn(-2.0, Dz);
+        // 2 D.x_i + |D|^2 = D.(2 x_i + D)
+        R[u].cp = __fma_rn(Dx, __fma_rn(2.0, xyi.x, Dx), __fma_rn(Dy, __fma_rn(2.0, xyi.y, Dy), __dmul_rn(Dz, __fma_rn(2.0, zi, Dz))));
         R[u].h = p.hh[i];
         R[u].acc = 0.0;
         R[u].m = 0x7fffffff;
@@ -256,10 +291,11 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
                     const double2 a0 = st.xy[j0 + jj], a1 = st.xy[j0 + jj + 1];
                     const double2 b0 = st.zq[j0 + jj], b1 = st.zq[j0 + jj + 1];
                     const double h0 = UNIFORM ? 0.0 : st.h[j0 + jj], h1 = UNIFORM ? 0.0 : st.h[j0 + jj + 1];
+                    const double n0 = st.n[j0 + jj], n1 = st.n[j0 + jj + 1];
 #pragma unroll
                     for (int u = 0; u < ROWS; ++u) {
-                        const int k0 = pair_eval<UNIFORM>(R[u], a0, b0, h0);
-                        const int k1 = pair_eval<UNIFORM>(R[u], a1, b1, h1);
+                        const int k0 = pair_eval_g<UNIFORM>(R[u], a0, b0, n0, h0);
+                        const int k1 = pair_eval_g<UNIFORM>(R[u], a1, b1, n1, h1);
                         R[u].m = __vimin3_s32(R[u].m, k0, k1);
                     }
                 }
@@ -373,8 +409,11 @@ __device__ __forceinline__ void chain_publisher(const PArgs& a, PShared& sh) {
             const unsigned fl = ho.out_flags[lane];
             const double dE = ho.out_dE[lane];
             if (fl & kFlagAccept) {
-                p.xy[i] = ho.txy[lane];
-                p.zq[i].x = ho.tz[lane];
+                const double2 t2 = ho.txy[lane];
+                const double tz = ho.tz[lane];
+                p.xy[i] = t2;
+                p.zq[i].x = tz;
+                p.nn[i] = dist2(t2.x, t2.y, tz);
                 e_lane = __dadd_rn(e_lane, dE);
             }
             p.log_dE[i] = dE;
