@@ -136,6 +136,13 @@ int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_
  * items fetched.  Synchronises. */
 int mc_debug_counters(mc_handle* h, int64_t* out16_host);
 
+/* Host-only check of the persistent kernel's work decomposition (no GPU needed): enumerates, for every
+ * chunk of 256 * rows_per_thread rows of an N-particle system, the FAR-L, FAR-U, MID, FIX and DIAG
+ * items exactly as the kernel slices them (far_cols = target columns per FAR item, far_workers = the
+ * number the item counts are rounded to, 0 = no rounding) and verifies that every column is covered
+ * exactly once per chunk.  out4_host = {items, violations, widest item in columns, urgent items}. */
+int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers, int64_t* out4_host);
+
 /* Diagnostics: copies the first n ints of the persistent kernel's scheduling state (ticket
  * counters, progress counter, per-chunk completion counters) to the host on a stream of its own,
  * without waiting for the handle's stream (usable while a sweep is running). */

@@ -22,7 +22,7 @@ EXPORTS = (
     "mc_workspace_bytes", "mc_init", "mc_sweep", "mc_energy", "mc_energy_dev", "mc_pair_hist", "mc_sweep_host",
     "mc_sweep_timed",
     "mc_get_positions", "mc_set_positions", "mc_get_sweep_index", "mc_set_sweep_index", "mc_get_stats",
-    "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option", "mc_debug_counters", "mc_debug_peek",
+    "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option", "mc_debug_counters", "mc_debug_peek", "mc_plan_check",
     "mc_get_launch_count",
 )
 
@@ -72,6 +72,7 @@ def load_library() -> C.CDLL:
     lib.mc_get_launch_count.argtypes = [vp, C.POINTER(u64)]
     lib.mc_debug_counters.argtypes = [vp, C.POINTER(C.c_int64)]
     lib.mc_debug_peek.argtypes = [vp, C.POINTER(C.c_int32), C.c_int]
+    lib.mc_plan_check.argtypes = [i64, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64)]
     for name in EXPORTS:
         if name not in ("mc_workspace_bytes", "mc_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -94,6 +95,13 @@ def _dev_f64(t, shape, device):
 # ---- functions with the C ABI's names ----------------------------------------------------------
 def mc_workspace_bytes(N: int) -> int:
     return int(load_library().mc_workspace_bytes(int(N)))
+
+
+def mc_plan_check(N: int, rows_per_thread: int, far_cols: int, far_workers: int) -> dict:
+    """Host-only check that the persistent kernel's items cover every column exactly once per chunk."""
+    out = (C.c_int64 * 4)()
+    _check(load_library().mc_plan_check(int(N), int(rows_per_thread), int(far_cols), int(far_workers), out))
+    return {"items": out[0], "violations": out[1], "max_item_cols": out[2], "urgent": out[3]}
 
 
 def mc_measure_fp64_peak(millis: float = 50.0) -> float:

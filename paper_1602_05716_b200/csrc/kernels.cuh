@@ -108,7 +108,7 @@ struct __align__(16) ColStage {
 // slice boundaries in the virtual column space: multiples of 8, so that every staged segment
 // holds a multiple of 8 columns (gap and range boundaries are multiples of 32) and the inner
 // loop needs no tail
-__device__ __forceinline__ int slice_bound(int ncols, int nslices, int sl) {
+__host__ __device__ __forceinline__ int slice_bound(int ncols, int nslices, int sl) {
     return (int)(((long long)(ncols >> 3) * sl) / nslices) << 3;
 }
 

@@ -2,6 +2,7 @@
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -fmad=false -shared -Xcompiler -fPIC
 #include "../../include/mcb200.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -714,6 +715,47 @@ int mc_debug_counters(mc_handle* h, int64_t* out16_host) {
     if (!h || !out16_host) return fail(MC_EINVAL, "null argument");
     CUDA_TRY(cudaMemcpyAsync(out16_host, h->ws + h->L.dbg, 16 * 8, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return MC_OK;
+}
+
+int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers, int64_t* out4_host) {
+    if (N < 1 || N > (int64_t)1 << 30 || !out4_host) return fail(MC_EINVAL, "bad argument");
+    if (rows_per_thread != 1 && rows_per_thread != 2 && rows_per_thread != 4) return fail(MC_EINVAL, "rows_per_thread must be 1, 2 or 4");
+    if (far_cols < 8 || far_cols % 8 || far_workers < 0) return fail(MC_EINVAL, "far_cols must be a positive multiple of 8, far_workers >= 0");
+    const int Np = padded(N), C = 256 * rows_per_thread, nchunks = (Np + C - 1) / C;
+    int64_t items = 0, violations = 0, max_item_cols = 0, urgent = 0;
+    std::vector<int> cover((size_t)Np / 8);
+    for (int c = 0; c < nchunks; ++c) {
+        const int row0 = c * C, nrows = chunk_rows(Np, C, c);
+        std::fill(cover.begin(), cover.end(), 0);
+        auto mark = [&](int col0, int ncol) {
+            if (col0 < 0 || ncol <= 0 || col0 % 8 || ncol % 8 || col0 + ncol > Np) { ++violations; return; }
+            for (int k = col0 / 8; k < (col0 + ncol) / 8; ++k) ++cover[k];
+            max_item_cols = std::max<int64_t>(max_item_cols, ncol);
+            ++items;
+        };
+        // FAR-L and FAR-U items, as the kernel slices them
+        for (int pass = 0; pass < 2; ++pass) {
+            const int cb = pass == 0 ? 0 : row0 + nrows;
+            const int ncols = pass == 0 ? farL_cols(C, c) : farU_cols(Np, C, c);
+            const int nf = far_slices(ncols, far_cols, far_workers);
+            if ((ncols > 0) != (nf > 0)) ++violations;
+            for (int k = 0; k < nf; ++k) {
+                const int v0 = slice_bound(ncols, nf, k), v1 = slice_bound(ncols, nf, k + 1);
+                mark(cb + v0, v1 - v0);
+            }
+            if (nf > 0 && slice_bound(ncols, nf, nf) != ncols) ++violations;
+        }
+        // urgent items: MID (chunk c-2), FIX (chunk c-1)
+        if (c >= 2) for (int j = 0; j < C / kMidCols; ++j) { mark(row0 - 2 * C + j * kMidCols, kMidCols); ++urgent; }
+        if (c >= 1) for (int j = 0; j < C / kFixCols; ++j) { mark(row0 - C + j * kFixCols, kFixCols); ++urgent; }
+        if (urgent_items(C, c) != (c >= 2 ? C / kMidCols : 0) + (c >= 1 ? C / kFixCols : 0)) ++violations;
+        // DIAG covers the chunk's own columns
+        for (int k = row0 / 8; k < (row0 + nrows) / 8; ++k) ++cover[k];
+        items += diag_items(nrows);
+        for (int k = 0; k < Np / 8; ++k) violations += cover[k] != 1;
+    }
+    out4_host[0] = items; out4_host[1] = violations; out4_host[2] = max_item_cols; out4_host[3] = urgent;
     return MC_OK;
 }
 

@@ -143,3 +143,15 @@ def test_reference_arm_prints_one_json_line():
     assert line["impl"] == "reference" and line["value"] > 1e5 and line["unit"] == "pair_evals/s"
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+@pytest.mark.parametrize("N", [1, 2, 31, 33, 255, 257, 512, 1023, 1025, 4096, 16383, 65536, 100001])
+@pytest.mark.parametrize("rows", [1, 2, 4])
+def test_persistent_kernel_items_cover_every_column_exactly_once(N, rows):
+    """Host logic of csrc/persist.cuh: FAR-L + FAR-U + MID + FIX + DIAG partition the N columns of every chunk
+    (Eq. 2: each partner enters a trial's sum exactly once)."""
+    from paper_1602_05716_b200.binding import mc_plan_check
+    for far_cols, workers in ((8, 0), (64, 0), (256, 290), (256, 7), (1024, 290), (65536, 3)):
+        r = mc_plan_check(N, rows, far_cols, workers)
+        assert r["violations"] == 0, (N, rows, far_cols, workers, r)
+        assert r["items"] > 0
