@@ -320,7 +320,7 @@ def run_ours(args, w):
         "achieved": 2.0 * achieved_instr / 1e12, "peak": 2.0 * peak_instr / 1e12, "unit": "TFLOP/s",
         "frac": achieved_instr / peak_instr, "traffic": read_measured_traffic(),
         "note": ("FP64 plain-ALU pipe; algorithmic count: 27 FP64-pipe instructions per pair evaluation (SURVEY.md "
-                 "8(d)), one FMA (2 flop) each; the kernel executes 22 per pair; peak = 64 lanes/SM x SMs x max SM "
+                 "8(d)), one FMA (2 flop) each; the kernel executes 20 per pair; peak = 64 lanes/SM x SMs x max SM "
                  "clock (derived, DESIGN.md); no FP64 entry in MEASURED_PEAKS.json"),
         "launches_per_sweep": bulk_launches, "avg_launch_ms": bulk_ms / max(1, bulk_launches),
         "pairs_per_launch": bulk_pairs / max(1, bulk_launches),

@@ -27,6 +27,10 @@ constexpr int kFixCols = 16;                   // columns per FIX item (columns 
 constexpr int kMidCols = 32;                   // columns per MID item (columns of chunk c-2)
 constexpr int kRing = 4;                       // hand-off ring depth of the chain CTA
 constexpr int kHelpers = 6;
+#ifndef MCB_COLS_PER_ITER
+#define MCB_COLS_PER_ITER 4
+#endif
+constexpr int kColsPerIter = MCB_COLS_PER_ITER;   // columns per iteration of the pair loop (2 pairs of rows x columns in flight per row)
 
 // scheduling state in global memory; zeroed by k_trial at the start of every sweep
 // (hot words 128 bytes apart, so that polling one does not slow down atomics on another)
@@ -285,9 +289,9 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
         const ColStage& st = sh.u.w.stage[s];
         if (warp_live) {
 #pragma unroll 1
-            for (int j0 = 0; j0 < cnt; j0 += 4) {     // cnt is a multiple of 8
+            for (int j0 = 0; j0 < cnt; j0 += kColsPerIter) {     // cnt is a multiple of 8
 #pragma unroll
-                for (int jj = 0; jj < 4; jj += 2) {
+                for (int jj = 0; jj < kColsPerIter; jj += 2) {
                     const double2 a0 = st.xy[j0 + jj], a1 = st.xy[j0 + jj + 1];
                     const double2 b0 = st.zq[j0 + jj], b1 = st.zq[j0 + jj + 1];
                     const double h0 = UNIFORM ? 0.0 : st.h[j0 + jj], h1 = UNIFORM ? 0.0 : st.h[j0 + jj + 1];
