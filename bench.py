@@ -63,13 +63,17 @@ def fp64_nominal_peak(num_sms: int, sm_mhz: float) -> float:
 
 
 def read_measured_traffic():
-    """DRAM bytes per k_bulk launch from the committed ncu --set full summary, or None."""
-    path = os.path.join(ROOT, "profiles", "k_bulk_dram_traffic.json")
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+    path = os.path.join(ROOT, "profiles", "r01c_k_sweep_traffic.csv")
     try:
         with open(path) as f:
-            return json.load(f).get("dram_bytes_per_launch")
-    except (OSError, ValueError):
-        return None
+            for line in f:
+                parts = line.strip().split(",")
+                if parts[0] == "dram_bytes_per_launch":
+                    return float(parts[2])
+    except (OSError, ValueError, IndexError):
+        pass
+    return None
 
 
 class ClockSampler:
