@@ -288,8 +288,7 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
         mbar_wait_wd(wd, &sh.full_bar[s], (k / kStages) & 1);
         const ColStage& st = sh.u.w.stage[s];
         if (warp_live) {
-#pragma unroll 1
-            for (int j0 = 0; j0 < cnt; j0 += kColsPerIter) {     // cnt is a multiple of 8
+            auto cols = [&](int j0) {
 #pragma unroll
                 for (int jj = 0; jj < kColsPerIter; jj += 2) {
                     const double2 a0 = st.xy[j0 + jj], a1 = st.xy[j0 + jj + 1];
@@ -303,6 +302,13 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
                         R[u].m = __vimin3_s32(R[u].m, k0, k1);
                     }
                 }
+            };
+            if (cnt == kColTile) {   // full stage: constant trip count
+#pragma unroll 1
+                for (int j0 = 0; j0 < kColTile; j0 += kColsPerIter) cols(j0);
+            } else {
+#pragma unroll 1
+                for (int j0 = 0; j0 < cnt; j0 += kColsPerIter) cols(j0);     // cnt is a multiple of 8
             }
         }
         __syncwarp();
@@ -468,7 +474,7 @@ namespace mcb {
 // the chain CTA (a3/a4): Alg. 4; accept iff no veto and
 // l_B q_i sum + ln u < 0 (Eq. 1 in log form, strict; readings G3, G4)
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ void chain_cta(const PArgs& a, PShared& sh) {
+__device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const Params& p = a.p;
     const int C = a.C;
@@ -651,7 +657,7 @@ __device__ __forceinline__ int ld_relaxed(const int* p) {
     return v;
 }
 
-__device__ __forceinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near, int* item) {
+__device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near, int* item) {
     const int C = a.C, GPC = C / kGroup, nfix = C / kFixCols, nmid = C / kMidCols;
     const int total_urgent = a.nchunks >= 2 ? nfix + (a.nchunks - 2) * (nfix + nmid) : 0;
     int* sy = a.sy;
@@ -693,6 +699,17 @@ __device__ __forceinline__ void fetch_item(const PArgs& a, Cursors& cur, bool ne
         if (l_done && u_done && d_done && u >= total_urgent) { item[0] = kItemExit; return; }
         __nanosleep(near ? 400 : 200);
     }
+}
+
+// DIAG item k of chunk c: 8 units (row tile, column tile), one per warp
+__device__ __noinline__ void diag_item(const PArgs& a, PShared& sh, int c, int k, int row0, int nrows) {
+    const int warp = threadIdx.x >> 5;
+    const ChunkBufs B = chunk_bufs(a, c);
+    Params pc = a.p;
+    pc.chunk = a.C;
+    pc.Dblk = B.Dblk; pc.OVold = B.OVold; pc.OVnew = B.OVnew;
+    diag_unit<true>(pc, row0, nrows, k * 8 + warp, sh.u.w.cxy[warp], sh.u.w.czq[warp], sh.u.w.ctxy[warp],
+                    sh.u.w.ch[warp], sh.u.w.ctz[warp]);
 }
 
 template <int ROWS, bool UNIFORM>
@@ -759,36 +776,26 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
         const long long t_item = clock64();
         if (type == kItemExit) break;
         const int row0 = c * C, nrows = chunk_rows(p.Np, C, c);
-        int* counter;
         if (type == kItemDiag) {
-            if (warp < 8) {
-                const ChunkBufs B = chunk_bufs(a, c);
-                Params pc = p;
-                pc.chunk = C;
-                pc.Dblk = B.Dblk; pc.OVold = B.OVold; pc.OVnew = B.OVnew;
-                diag_unit<true>(pc, row0, nrows, k * 8 + warp, sh.u.w.cxy[warp], sh.u.w.czq[warp], sh.u.w.ctxy[warp],
-                                sh.u.w.ch[warp], sh.u.w.ctz[warp]);
-            }
-            counter = sy_diag_done(a) + c;
-        } else if (type == kItemFarL || type == kItemFarU) {
-            // columns [cb, cb + ncols): before chunk c-1 (L) or after chunk c (U); probe: all but the chunk's own
-            const bool probe = a.mode == 1;
-            const int cb = (type == kItemFarL || probe) ? 0 : row0 + nrows;
-            const int ncols = probe ? probe_cols(p.Np, C, c) : type == kItemFarL ? farL_cols(C, c) : farU_cols(p.Np, C, c);
-            const int nf = far_slices(ncols, a.farcols, a.nfar);
-            const int v0 = slice_bound(ncols, nf, k), v1 = slice_bound(ncols, nf, k + 1);
-            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, probe ? row0 : cb, probe ? row0 + nrows : cb, v0, v1);
-            counter = sy_far_done(a) + c;
-        } else if (type == kItemMid) {
-            const int cb = row0 - 2 * C + k * kMidCols;
-            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, cb, cb, 0, kMidCols);
-            counter = sy_fix_done(a) + c;
+            if (warp < 8) diag_item(a, sh, c, k, row0, nrows);
         } else {
-            const int cb = row0 - C + k * kFixCols;
-            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, cb, cb, 0, kFixCols);
-            counter = sy_fix_done(a) + c;
+            // one call site for the pair loop: the item's column space [cb, cb + ...) minus [g0, g1), columns [v0, v1) of it
+            int cb, g0, g1, v0, v1;
+            if (type == kItemFarL || type == kItemFarU) {
+                // before chunk c-2 (L) or after chunk c (U); probe: all columns but the chunk's own
+                const bool probe = a.mode == 1;
+                cb = (type == kItemFarL || probe) ? 0 : row0 + nrows;
+                const int ncols = probe ? probe_cols(p.Np, C, c) : type == kItemFarL ? farL_cols(C, c) : farU_cols(p.Np, C, c);
+                const int nf = far_slices(ncols, a.farcols, a.nfar);
+                v0 = slice_bound(ncols, nf, k); v1 = slice_bound(ncols, nf, k + 1);
+                g0 = probe ? row0 : cb; g1 = probe ? row0 + nrows : cb;
+            } else {
+                const int w = type == kItemMid ? kMidCols : kFixCols;
+                cb = row0 - (type == kItemMid ? 2 : 1) * C + k * w;
+                g0 = g1 = cb; v0 = 0; v1 = w;
+            }
+            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, g0, g1, v0, v1);
         }
-        (void)counter;
         __syncthreads();
         if (tid == 0) {
             // completion counter of this item's queue and chunk (item[] is stable until the next fetch)
