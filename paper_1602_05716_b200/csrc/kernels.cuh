@@ -671,7 +671,7 @@ __global__ void k_check_particles(Params p, const double* d) {
 // ------------------------------------------------------------------------------------------
 // a5: from-scratch energy (and the overlap check of mc_init): E = l_B sum_{i<j} q_i q_j / r_ij.
 // The upper triangle is cut into units of 1024 rows x 1024 columns (4 column tiles of 256); one CTA
-// per unit, 4 rows per thread, columns staged through shared memory, 12 FP64-pipe instructions per
+// per unit, 4 rows per thread, columns staged through shared memory, 10 FP64-pipe instructions per
 // pair.  Units on the diagonal test j > i per pair.  Every CTA reduces its rows in a fixed order and
 // writes one partial; k_energy_reduce adds the partials in index order.
 // ------------------------------------------------------------------------------------------
@@ -687,7 +687,7 @@ __host__ __device__ inline int energy_units(int Np) {
 template <bool CHECK>
 __global__ void __launch_bounds__(256, 2) k_energy(Params p, double* part) {
     __shared__ double2 sxy[kETile], szq[kETile];
-    __shared__ double sh[kETile];
+    __shared__ double sh[kETile], sn[kETile];
     __shared__ double red[8];
     const int tid = threadIdx.x;
     // unit -> (row block rb, column block cb >= rb)
@@ -699,7 +699,10 @@ __global__ void __launch_bounds__(256, 2) k_energy(Params p, double* part) {
         ++rb;
     }
     const int cb = rb + unit;
-    double x[kERows], y[kERows], z[kERows], q[kERows], h[kERows], acc[kERows];
+    // off the diagonal: r^2 = |x_i|^2 + |x_j|^2 - 2 x_i.x_j (1 DADD + 3 DFMA; |x|^2 is kept per particle, p.nn),
+    // 10 FP64-pipe instructions per pair; on the diagonal and in the overlap check of mc_init the
+    // differences are formed explicitly (reading G11's evaluation order)
+    double x[kERows], y[kERows], z[kERows], q[kERows], h[kERows], nn[kERows], acc[kERows];
     int bad = 0;
 #pragma unroll
     for (int u = 0; u < kERows; ++u) {
@@ -709,23 +712,31 @@ __global__ void __launch_bounds__(256, 2) k_energy(Params p, double* part) {
         const double2 zq = live ? p.zq[i] : make_double2(0.0, 0.0);
         x[u] = xy.x; y[u] = xy.y; z[u] = zq.x; q[u] = zq.y;
         h[u] = live ? p.hh[i] : 0.0;
+        nn[u] = live ? p.nn[i] : 9.0e18;
         acc[u] = 0.0;
     }
+    const bool diagonal = cb == rb;
+    double mx[kERows], my[kERows], mz[kERows];
+#pragma unroll
+    for (int u = 0; u < kERows; ++u) { mx[u] = __dmul_rn(-2.0, x[u]); my[u] = __dmul_rn(-2.0, y[u]); mz[u] = __dmul_rn(-2.0, z[u]); }
     for (int ct = 0; ct < kEBlock / kETile; ++ct) {
         const int j0 = cb * kEBlock + ct * kETile;
         if (j0 >= p.Np) break;
         const int cnt = min(kETile, p.Np - j0);
         __syncthreads();
-        if (tid < cnt) { sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; if (CHECK) sh[tid] = p.hh[j0 + tid]; }
+        if (tid < cnt) {
+            sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; sn[tid] = p.nn[j0 + tid];
+            if (CHECK) sh[tid] = p.hh[j0 + tid];
+        }
         __syncthreads();
-        const bool diagonal = cb == rb;
         if (!diagonal && !CHECK) {
 #pragma unroll 2
             for (int j = 0; j < cnt; ++j) {
                 const double2 a = sxy[j], b = szq[j];
+                const double nj = sn[j];
 #pragma unroll
                 for (int u = 0; u < kERows; ++u) {
-                    const double r2 = dist2(__dadd_rn(x[u], -a.x), __dadd_rn(y[u], -a.y), __dadd_rn(z[u], -b.x));
+                    const double r2 = __fma_rn(mx[u], a.x, __fma_rn(my[u], a.y, __fma_rn(mz[u], b.x, __dadd_rn(nn[u], nj))));
                     acc[u] = __fma_rn(b.y, rsqrt_fast(r2), acc[u]);
                 }
             }
