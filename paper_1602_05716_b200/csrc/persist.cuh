@@ -666,7 +666,7 @@ __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near,
         if ((it & 1023u) == 0u) wd_check(wd, global_ns());   // no time limit of its own: leaves when another wait gave up
         // one round trip: five independent loads
         const int tl = ld_relaxed(sy + kSyTicket), tu = ld_relaxed(sy + kSyTicketU), td = ld_relaxed(sy + kSyDTicket);
-        const int u = ld_relaxed(sy + kSyUTicket), groups = ld_relaxed(sy + kSyGroups);
+        const int u = ld_relaxed(sy + kSyUTicket), groups = ld_acquire(sy + kSyGroups);   // acquire: what the chain published
         bool got = false, l_done = true, u_done = true, d_done = false;
         if (a.mode == 1) {
             got = try_queue<QU>(a, cur.u, tu, groups, item, u_done);
@@ -692,10 +692,7 @@ __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near,
         if (!got) got = try_queue<QD>(a, cur.d, td, groups, item, d_done);
         if (!got && !near) got = try_queue<QL>(a, cur.l, tl, groups, item, l_done);
         if (!got && !near) got = try_queue<QU>(a, cur.u, tu, groups, item, u_done);
-        if (got) {
-            __threadfence();   // acquire: what the chain published before the progress value read above
-            return;
-        }
+        if (got) return;
         if (l_done && u_done && d_done && u >= total_urgent) { item[0] = kItemExit; return; }
         __nanosleep(near ? 400 : 200);
     }
