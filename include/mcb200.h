@@ -35,7 +35,7 @@ extern "C" {
 #endif
 
 #define MC_OK 0
-#define MC_EINVAL (-1)   /* bad argument, non-finite input, d <= 0, R <= 0, l_B < 0, max_disp < 0 */
+#define MC_EINVAL (-1)   /* bad argument, non-finite input, d <= 0, R <= 0, l_B < 0, max_disp < 0, R/d_min > 2e4 */
 #define MC_EOVERLAP (-2) /* two ions overlap in the initial configuration                          */
 #define MC_EOUTSIDE (-3) /* an ion sticks out of the cavity in the initial configuration           */
 #define MC_ENOSPACE (-4) /* workspace too small                                                    */

@@ -25,6 +25,7 @@ struct DevState {
     int err;        // validation result (0 ok, MC_E* otherwise)
     int d_differs;  // set by k_check_particles if not all diameters are equal
     int stall;      // set by the persistent sweep kernel's watchdog (a wait exceeded its time limit)
+    unsigned long long dmin_bits;   // bit pattern of the smallest diameter (k_check_particles; ~0 before)
 };
 
 // ---------------------------------------------------------------------------------------------

@@ -666,6 +666,7 @@ __global__ void k_check_particles(Params p, const double* d) {
     }
     if (err) atomicMin(&p.st->err, err == -1 ? -1000 : err);  // EINVAL outranks the others
     if (di != d[0]) p.st->d_differs = 1;
+    if (di > 0.0) atomicMin(&p.st->dmin_bits, (unsigned long long)__double_as_longlong(di));   // positive doubles order as integers
 }
 
 // ------------------------------------------------------------------------------------------

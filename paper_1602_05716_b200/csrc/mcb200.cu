@@ -384,6 +384,11 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     cudaError_t e = cudaMemsetAsync(w, 0, L.total, h->stream);
     if (e != cudaSuccess) return bail(fail(MC_ECUDA, std::string("memset: ") + cudaGetErrorString(e)));
     const int nb = (p.Np + 255) / 256;
+    {
+        const unsigned long long ones = ~0ull;
+        e = cudaMemcpyAsync(&p.st->dmin_bits, &ones, sizeof(ones), cudaMemcpyHostToDevice, h->stream);
+        if (e != cudaSuccess) return bail(fail(MC_ECUDA, std::string("init: ") + cudaGetErrorString(e)));
+    }
     k_pack<<<nb, 256, 0, h->stream>>>(p, pos_dev, charges_dev, diameters_dev);
     k_check_particles<<<nb, 256, 0, h->stream>>>(p, diameters_dev);
     h->launches += 2;
@@ -396,6 +401,14 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return bail(fail(MC_ECUDA, std::string("init: ") + cudaGetErrorString(e)));
     h->all_d_equal = st.d_differs == 0;
+    if (st.err == 0) {
+        // the sweep kernels form r^2 from |x_i|^2 + |x_j|^2 - 2 x_i.x_j and re-examine a veto exactly only
+        // within 2^-16 relative of the contact distance: that needs (R / d_min)^2 * 2^-50 << 2^-16
+        double dmin;
+        std::memcpy(&dmin, &st.dmin_bits, sizeof(dmin));
+        if (!(dmin > 0) || cavity_R / dmin > 2.0e4)
+            return bail(fail(MC_EINVAL, "cavity_R / smallest diameter exceeds 2e4: outside the range the FP64 veto band covers"));
+    }
     h->uniform_d = h->allow_uniform && h->all_d_equal;
     if (st.err != 0) {
         if (st.err <= -1000) return bail(fail(MC_EINVAL, "non-finite input or diameter <= 0"));

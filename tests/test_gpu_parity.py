@@ -322,6 +322,10 @@ def test_init_validation_errors():
     assert e.value.code == MC_EINVAL
     # contact is allowed (G6, G7): touching the wall and each other
     MCSystem(np.array([[-0.5, 0.5], [0.0, 0.0], [0.0, 0.0]]), q, d, 1.0, 1.68, 0.1, 1)
+    # the range the FP64 veto band covers: cavity_R / d_min <= 2e4
+    with pytest.raises(MCError) as e:
+        MCSystem(ok, q, np.array([1.0, 1.0e-4]), 5.0, 1.68, 0.1, 1)
+    assert e.value.code == MC_EINVAL
 
 
 def test_workspace_too_small_and_bad_arguments_through_the_raw_abi():
