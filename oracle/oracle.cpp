@@ -295,17 +295,21 @@ int oracle_energy(void* hp, double* E) {
 
 // hist [2][2][nbins] and n_centres [2] are accumulators (added to).  Species 0 if
 // q > 0 else 1.  Ordered pairs (centre i in the bulk, any partner j != i).
+// With more than one thread (oracle_set_threads) the centres are shared out over
+// threads, each counting into a private copy that is added at the end: integer
+// counts, so the result is the serial one whatever the order (reading G17).
 int oracle_pair_hist(void* hp, double bin_width, int nbins, double centre_rmax, uint64_t* hist,
                      uint64_t* n_centres) {
     if (!hp || !hist || !n_centres || !(bin_width > 0) || nbins < 1) return ORACLE_EINVAL;
     const Handle& h = *(Handle*)hp;
     const double inv_w = 1.0 / bin_width;
     const double c2 = centre_rmax * centre_rmax;
-    for (int64_t i = 0; i < h.N; ++i) {
+    // all partners of one centre, counted into hs / ns
+    auto centre = [&](int64_t i, uint64_t* hs, uint64_t* ns) {
         const double rr = std::fma(h.z[i], h.z[i], std::fma(h.y[i], h.y[i], h.x[i] * h.x[i]));
-        if (!(rr <= c2)) continue;
+        if (!(rr <= c2)) return;
         const int si = h.q[i] > 0 ? 0 : 1;
-        n_centres[si] += 1;
+        ns[si] += 1;
         for (int64_t j = 0; j < h.N; ++j) {
             if (j == i) continue;
             const double dx = h.x[i] - h.x[j], dy = h.y[i] - h.y[j], dz = h.z[i] - h.z[j];
@@ -314,7 +318,24 @@ int oracle_pair_hist(void* hp, double bin_width, int nbins, double centre_rmax, 
             const double fb = std::floor(r * inv_w);
             if (fb < (double)nbins) {
                 const int sj = h.q[j] > 0 ? 0 : 1;
-                hist[((size_t)si * 2 + sj) * (size_t)nbins + (size_t)fb] += 1;
+                hs[((size_t)si * 2 + sj) * (size_t)nbins + (size_t)fb] += 1;
+            }
+        }
+    };
+    if (h.threads <= 1) {
+        for (int64_t i = 0; i < h.N; ++i) centre(i, hist, n_centres);
+    } else {
+#pragma omp parallel num_threads(h.threads)
+        {
+            std::vector<uint64_t> hs((size_t)4 * nbins, 0);
+            uint64_t ns[2] = {0, 0};
+#pragma omp for schedule(dynamic, 64)
+            for (int64_t i = 0; i < h.N; ++i) centre(i, hs.data(), ns);
+#pragma omp critical
+            {
+                for (size_t k = 0; k < hs.size(); ++k) hist[k] += hs[k];
+                n_centres[0] += ns[0];
+                n_centres[1] += ns[1];
             }
         }
     }

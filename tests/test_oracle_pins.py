@@ -368,3 +368,56 @@ def test_pair_hist_against_numpy():
     # accumulates
     hist2, nc2 = o.pair_hist(bw, nb, crm, hist.copy(), nc.copy())
     assert np.array_equal(hist2, 2 * ref) and np.array_equal(nc2, 2 * nc)
+
+
+def test_pair_hist_hand_placed_example():
+    """A configuration whose histogram can be written down by hand (reading G17):
+    known distances on and off bin edges, both species, one centre just inside and one just outside
+    centre_rmax.  Pins the [centre species][partner species] order, the bin edges (left-closed:
+    bin k = [k w, (k+1) w)), the <= at centre_rmax, the dropped bins >= nbins and the ordered-pair count."""
+    # ions on the x axis: index, x, charge
+    #   0: 0.0   +     1: 1.5   -     2: 3.0   +     3: 6.0   -      4: (0, 2.0, 0) -
+    pos = np.array([[0.0, 1.5, 3.0, 6.0, 0.0],
+                    [0.0, 0.0, 0.0, 0.0, 2.0],
+                    [0.0, 0.0, 0.0, 0.0, 0.0]])
+    q = np.array([1.0, -1.0, 1.0, -1.0, -1.0])
+    d = np.full(5, 1.0)
+    o = Oracle(pos, q, d, 50.0, 1.68, 0.1, 1)
+    bw, nb = 0.5, 8                     # bins [0,.5) [.5,1) ... [3.5,4.0); r >= 4.0 is dropped
+    # centre_rmax = 3.0: ions 0 (r=0), 1 (1.5), 2 (3.0, ON the limit: counts, <=), 4 (2.0) are centres; 3 (6.0) is not
+    hist, nc = o.pair_hist(bw, nb, 3.0)
+    assert list(nc) == [2, 2]           # centres: + {0, 2}, - {1, 4}
+    exp = np.zeros((2, 2, nb), dtype=np.uint64)
+    P, M = 0, 1
+    def add(a, b, r):
+        k = int(np.floor(r / bw))
+        if k < nb:
+            exp[a, b, k] += 1
+    # centre 0 (+): partners 1 (-, 1.5 -> bin 3 exactly on the edge 1.5 = 3 w), 2 (+, 3.0 -> bin 6), 3 (-, 6.0 dropped), 4 (-, 2.0 -> bin 4)
+    add(P, M, 1.5); add(P, P, 3.0); add(P, M, 6.0); add(P, M, 2.0)
+    # centre 1 (-): 0 (+, 1.5), 2 (+, 1.5), 3 (-, 4.5 dropped), 4 (-, 2.5 -> bin 5)
+    add(M, P, 1.5); add(M, P, 1.5); add(M, M, 4.5); add(M, M, 2.5)
+    # centre 2 (+): 0 (+, 3.0), 1 (-, 1.5), 3 (-, 3.0 -> bin 6), 4 (-, sqrt(13) = 3.606 -> bin 7)
+    add(P, P, 3.0); add(P, M, 1.5); add(P, M, 3.0); add(P, M, np.sqrt(13.0))
+    # centre 4 (-): 0 (+, 2.0), 1 (-, 2.5), 2 (+, 3.606), 3 (-, sqrt(40) dropped)
+    add(M, P, 2.0); add(M, M, 2.5); add(M, P, np.sqrt(13.0)); add(M, M, np.sqrt(40.0))
+    assert np.array_equal(hist, exp), (hist, exp)
+    # written out: the table above in numbers
+    assert hist[P, M, 3] == 2 and hist[P, P, 6] == 2 and hist[P, M, 4] == 1 and hist[P, M, 6] == 1 and hist[P, M, 7] == 1
+    assert hist[M, P, 3] == 2 and hist[M, M, 5] == 2 and hist[M, P, 4] == 1 and hist[M, P, 7] == 1
+    assert hist.sum() == 13
+    # just inside the limit: ion 2 leaves the centres, nothing else changes
+    hist2, nc2 = o.pair_hist(bw, nb, 3.0 - 1e-12)
+    assert list(nc2) == [1, 2] and hist2.sum() == 13 - 4
+    # not symmetric in (centre, partner): ion 3 is a partner but never a centre
+    assert hist[P, M].sum() != hist[M, P].sum()
+
+
+def test_pair_hist_threaded_matches_serial():
+    w = W.scaled(W.CONFIGS[2], 900)
+    pos, q, d = w.arrays()
+    a = Oracle(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 2)
+    b = Oracle(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 2, threads=4)
+    ha, na = a.pair_hist(0.05, 60, 0.7 * w.cavity_R)
+    hb, nb_ = b.pair_hist(0.05, 60, 0.7 * w.cavity_R)
+    assert np.array_equal(ha, hb) and np.array_equal(na, nb_) and ha.sum() > 0
