@@ -34,6 +34,9 @@ UNIT = "pair_evals/s"
 FP64_INSTR_PER_PAIR = 27          # SURVEY.md 8(d) canonical count
 FP64_LANES_PER_SM = 64            # DFMA lanes per SM per clock (confirmed by mc_measure_fp64_peak)
 L2_FLUSH_BYTES = 256 << 20        # > 126 MB L2
+# FP64-pipe instructions the sweep kernel EXECUTES per pair, by pair-distance form (persist.cuh) and
+# (equal diameters, mixed diameters); the roofline fraction credits the canonical 27 whatever the form
+EXECUTED_FP64_PER_PAIR = {0: (20, 22), 1: (22, 24), 2: (25, 27)}
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -62,9 +65,13 @@ def fp64_nominal_peak(num_sms: int, sm_mhz: float) -> float:
     return FP64_LANES_PER_SM * num_sms * sm_mhz * 1e6
 
 
+TRAFFIC_FILE = os.path.join("profiles", "r02_k_sweep_traffic.csv")
+
+
 def read_measured_traffic():
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
-    path = os.path.join(ROOT, "profiles", "r01c_k_sweep_traffic.csv")
+    """DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of one
+    ``ncu --set full`` capture of this command, kept under profiles/), or None if there is no capture."""
+    path = os.path.join(ROOT, TRAFFIC_FILE)
     try:
         with open(path) as f:
             for line in f:
@@ -181,7 +188,8 @@ def run_reference(args, w):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_config(w, world=1, parallelism="cpu"),
             "sweeps_per_s": value / w.pair_evals_per_sweep,
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "note": "the plain scalar parity oracle as it stands, not a tuned CPU code"},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -275,9 +283,14 @@ def run_ours(args, w):
     pin_hist = torch.empty((2, 2, w.hist_nbins), dtype=torch.int64).pin_memory()
     pin_ncent = torch.empty(2, dtype=torch.int64).pin_memory()
 
+    e_run = [sysm.mc_get_stats()["E_running"]]
+    pin_in.copy_(torch.from_numpy(sysm.positions))              # the chain's current state, with its running energy
+
     def step_e2e():
         hist.zero_(); ncent.zero_()
-        _, st = sysm.mc_sweep_host(1, pin_in, pin_out)          # H2D positions, sweep, D2H positions + stats
+        # H2D positions (+ the running energy that belongs to them: no from-scratch pass), sweep, D2H positions + stats
+        _, st = sysm.mc_sweep_host(1, pin_in, pin_out, E_running_in=e_run[0])
+        e_run[0] = st["E_running"]
         sysm.mc_pair_hist(w.hist_bin_width, w.hist_nbins, w.hist_centre_rmax, hist, ncent)
         pin_hist.copy_(hist, non_blocking=True)
         pin_ncent.copy_(ncent, non_blocking=True)
@@ -285,7 +298,7 @@ def run_ours(args, w):
         pin_in.copy_(pin_out)                                   # the next step continues the chain
         return st, e
 
-    h2d = 3 * N * 8
+    h2d = 3 * N * 8 + 8
     d2h = 3 * N * 8 + 40 + 4 * w.hist_nbins * 8 + 16 + 8
     for _ in range(min(args.warmup, 3)):
         step_e2e()
@@ -306,13 +319,16 @@ def run_ours(args, w):
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel (k_bulk), timed live with an event pair around every launch ----
-    timed = sysm.mc_sweep_timed()
-    for _ in range(2):
-        t2 = sysm.mc_sweep_timed()
-        if t2["k_bulk"][0] < timed["k_bulk"][0]:
-            timed = t2
-    bulk_ms, bulk_launches, bulk_pairs = timed["k_bulk"]
+    # ---- roofline of the dominant kernel (k_sweep): CUDA events on the launching stream around its launch,
+    #      average over the launches of a timed region of its own (L2 flushed in between, as in the steps) ----
+    runs = []
+    for _ in range(max(3, min(args.steps, 10))):
+        flush.zero_()
+        runs.append(sysm.mc_sweep_timed())
+    timed = {k: (sum(r[k][0] for r in runs) / len(runs), runs[0][k][1], runs[0][k][2]) for k in runs[0]}
+    bulk_ms, bulk_launches, bulk_pairs = timed["k_sweep"]
+    form = sysm.mc_get_option("form")
+    executed = EXECUTED_FP64_PER_PAIR[form][0 if sysm.mc_get_option("uniform_path") else 1]
     prop = torch.cuda.get_device_properties(dev)
     sm_max = clocks["sm_max_mhz"] or 1965.0
     peak_instr = fp64_nominal_peak(prop.multi_processor_count, sm_max)
@@ -320,15 +336,20 @@ def run_ours(args, w):
     achieved_instr = bulk_pairs * FP64_INSTR_PER_PAIR / (bulk_ms * 1e-3) if bulk_ms > 0 else 0.0
     total_timed_ms = sum(v[0] for v in timed.values())
     roofline = {
-        "bound": "alu", "kernel": "k_sweep (persistent: the whole sweep in one launch)" if bulk_launches == 1 else "k_bulk",
+        "bound": "alu", "kernel": "k_sweep (persistent: the whole sweep in one cooperative launch)",
         "achieved": 2.0 * achieved_instr / 1e12, "peak": 2.0 * peak_instr / 1e12, "unit": "TFLOP/s",
         "frac": achieved_instr / peak_instr, "traffic": read_measured_traffic(),
-        "note": ("FP64 plain-ALU pipe; algorithmic count: 27 FP64-pipe instructions per pair evaluation (SURVEY.md "
-                 "8(d)), one FMA (2 flop) each; the kernel executes 20 per pair; peak = 64 lanes/SM x SMs x max SM "
-                 "clock (derived, DESIGN.md); no FP64 entry in MEASURED_PEAKS.json"),
+        "note": ("FP64 plain-ALU pipe; frac = ALGORITHMIC work / peak: 27 FP64-pipe instructions per pair evaluation "
+                 "(SURVEY.md 8(d)), one FMA (2 flop) each, against peak = 64 lanes/SM x SMs x max SM clock (derived, "
+                 "DESIGN.md section 4; MEASURED_PEAKS.json has no FP64 entry; the builder-measured DFMA rate of this "
+                 "run is beside it). The kernel EXECUTES fewer instructions per pair (executed_fp64_per_pair), so "
+                 "frac can exceed the pipe's own utilisation: pipe_utilisation_executed is that one"),
+        "executed_fp64_per_pair": executed, "pair_distance_form": ("gram", "diffw", "canon")[form],
+        "pipe_utilisation_executed": (bulk_pairs * executed / (bulk_ms * 1e-3) / measured_dfma) if bulk_ms > 0 else 0.0,
+        "traffic_source": TRAFFIC_FILE,
         "launches_per_sweep": bulk_launches, "avg_launch_ms": bulk_ms / max(1, bulk_launches),
         "pairs_per_launch": bulk_pairs / max(1, bulk_launches),
-        "measured_dfma_per_s": measured_dfma, "frac_of_measured_dfma": achieved_instr / measured_dfma,
+        "builder_measured_dfma_per_s": measured_dfma, "frac_of_builder_measured_dfma_peak": achieved_instr / measured_dfma,
         "kernel_share_of_serial_sweep": {k: v[0] / total_timed_ms for k, v in timed.items()},
         "serial_sweep_ms": total_timed_ms,
     }
@@ -345,6 +366,7 @@ def run_ours(args, w):
                                    f"OpenMP over j, {cores} threads)"),
                         "single_thread": {"value": cpu_one, "cores": 1,
                                           "sample": f"first {n_one} trials of sweep 0 ({s_one:.1f} s)"},
+                        "note": "the plain scalar parity oracle as it stands, not a tuned CPU code",
                         "paper_context": "paper: 440x over one Xeon core on Tesla K20 (PAPER.md:315)"}
 
     st = sysm.mc_get_stats()
@@ -371,6 +393,20 @@ def run_ours(args, w):
     return 0
 
 
+def spawn_replicas(n: int, argv: list, runner=None) -> int:
+    """``python bench.py --gpus N`` outside torchrun: start the N replicas itself, one process per GPU, the
+    way the driver does (torch.distributed.run on 127.0.0.1); rank 0 of them prints the JSON line."""
+    import socket
+    import subprocess
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
+    return (runner or subprocess.call)(cmd)
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -381,6 +417,8 @@ def main(argv=None):
     ap.add_argument("--skip-cpu-baseline", action="store_true",
                     help="leave out the oracle timing (profiling runs under ncu only)")
     args = ap.parse_args(argv)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        return spawn_replicas(args.gpus, list(sys.argv[1:] if argv is None else argv))
     from paper_1602_05716_b200 import workloads as W
     w = W.by_name(args.workload) if args.workload else W.HEADLINE
     if args.impl == "reference":

@@ -35,12 +35,14 @@ extern "C" {
 #endif
 
 #define MC_OK 0
-#define MC_EINVAL (-1)   /* bad argument, non-finite input, d <= 0, R <= 0, l_B < 0, max_disp < 0, R/d_min > 2e4 */
+#define MC_EINVAL (-1)   /* bad argument, non-finite input, d <= 0, R <= 0 or > 1e7, l_B < 0, max_disp < 0, R/d_min > 1e6 */
 #define MC_EOVERLAP (-2) /* two ions overlap in the initial configuration                          */
 #define MC_EOUTSIDE (-3) /* an ion sticks out of the cavity in the initial configuration           */
 #define MC_ENOSPACE (-4) /* workspace too small                                                    */
 #define MC_ECUDA (-5)    /* a CUDA runtime call failed, or no sm_100 device                        */
-#define MC_ESTALL (-6)   /* the sweep kernel's watchdog fired (a wait exceeded 2 s): state invalid  */
+#define MC_ESTALL (-6)   /* a sweep stalled (a wait of the sweep kernel exceeded "stall_ms"): the state is  \
+                            invalid and every later sweep is a no-op until mc_set_positions / mc_set_state;  \
+                            reported by every call that synchronises                                        */
 
 typedef struct mc_handle mc_handle;
 
@@ -65,7 +67,10 @@ size_t mc_workspace_bytes(int64_t N);
  *   workspace_dev/workspace_bytes: >= mc_workspace_bytes(N), 256-byte aligned.
  * Validates on the device (finite, d > 0, inside the wall, no overlapping pair: O(N^2)),
  * sets sweep index 0, E_running = from-scratch energy, counters 0.  Synchronises.
- * validate = 0 skips the O(N^2) overlap check and the energy (E_running = 0). */
+ * validate = 0 skips the O(N^2) overlap check and the energy (E_running = 0).
+ * Accuracy contract: per-trial dE within 1e-10 of max(|dE|, M_i) (reading G13) for any geometry
+ * with cavity_R <= 1e7 and cavity_R / d_min <= 1e6; the pair-distance form is chosen from
+ * cavity_R / d_min and max_disp / d_min (option "form"). */
 int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* charges_dev,
             const double* diameters_dev, double cavity_R, double bjerrum_length, double max_disp,
             uint64_t seed, void* workspace_dev, size_t workspace_bytes, void* stream, int validate);
@@ -90,21 +95,32 @@ int mc_pair_hist(mc_handle* h, double bin_width, int nbins, double centre_rmax,
                  uint64_t* hist_dev, uint64_t* n_centres_dev);
 
 /* Same n sweeps through HOST buffers (the end-to-end path): if pos_in_host != NULL it is
- * uploaded ([3][N]) and replaces the configuration as mc_set_positions does; after the sweeps
- * positions ([3][N]) and stats are downloaded into pos_out_host / stats_host (either may be
- * NULL).  Host buffers should be pinned for the copies to be asynchronous.  Synchronises. */
-int mc_sweep_host(mc_handle* h, int64_t n, const double* pos_in_host, double* pos_out_host,
-                  mc_stats* stats_host);
+ * uploaded ([3][N]) and replaces the configuration -- as mc_set_positions does (from-scratch
+ * energy, O(N^2/2)) if E_running_in == NULL, else with E_running := *E_running_in taken on trust
+ * (a caller that feeds back the positions and the E_running it just downloaded pays no extra
+ * pass).  After the sweeps positions ([3][N]) and stats are downloaded into pos_out_host /
+ * stats_host (either may be NULL).  Host buffers should be pinned for the copies to be
+ * asynchronous.  Synchronises. */
+int mc_sweep_host(mc_handle* h, int64_t n, const double* pos_in_host, const double* E_running_in,
+                  double* pos_out_host, mc_stats* stats_host);
 
-/* ---- accessors for parity tests, near-tie re-sync and checkpoint/resume ---- */
+/* ---- accessors for parity tests, near-tie re-sync and checkpoint/resume.  The state of a chain is
+ * the particle array (it is downloaded for analysis), the sweep counter that keys
+ * the random stream (reading G9) and the running energy that is monitored. ---- */
 int mc_get_positions(mc_handle* h, double* pos_dev_out /* [3][N] */);          /* enqueued */
-/* Replaces the configuration (not validated); E_running := from-scratch energy. Enqueued. */
+/* Replaces the configuration (not validated); E_running := from-scratch energy; clears a stall. Enqueued. */
 int mc_set_positions(mc_handle* h, const double* pos_dev /* [3][N] */);
+/* Checkpoint resume in one call: configuration (not validated), sweep index and running energy as
+ * saved from mc_get_positions / mc_get_sweep_index / mc_get_stats; no O(N^2) pass; clears a stall. Enqueued. */
+int mc_set_state(mc_handle* h, const double* pos_dev /* [3][N] */, uint64_t sweep_index, double E_running);
 int mc_get_sweep_index(mc_handle* h, uint64_t* s_host);                         /* synchronises */
 int mc_set_sweep_index(mc_handle* h, uint64_t s);                               /* enqueued */
-int mc_get_stats(mc_handle* h, mc_stats* stats_host);                           /* synchronises */
-/* Log of the last sweep: dE_dev [N] (k_B T; unspecified for overlap-vetoed trials) and
- * flags_dev [N]: bit0 accept, bit1 overlap veto, bit2 wall veto, bit3 near-tie.  Enqueued. */
+/* Counters since mc_init and the running energy (energy monitored during warm-up;
+ * vetoes are counted apart from energy rejections).  Synchronises. */
+int mc_get_stats(mc_handle* h, mc_stats* stats_host);
+/* Log of the last sweep (Alg. 4: one decision per particle): dE_dev [N] (k_B T;
+ * unspecified for overlap-vetoed trials, reading G14) and flags_dev [N]: bit0 accept, bit1 overlap
+ * veto, bit2 wall veto, bit3 near-tie.  Either may be NULL.  Enqueued. */
 int mc_get_trial_log(mc_handle* h, double* dE_dev, uint8_t* flags_dev);
 int mc_free(mc_handle* h);
 
@@ -116,17 +132,13 @@ const char* mc_last_error(void);
 int mc_measure_fp64_peak(void* stream, double millis, double* dfma_per_second_host);
 
 /* Diagnostics for the roofline: runs ONE sweep (it advances the chain exactly as mc_sweep(h, 1)
- * does, same kernels, same arguments, bit-identical result) with the kernels launched one after
- * the other on the handle's stream and a CUDA event pair around every launch.  Fills
- * ms_host[MC_NKERNELS] with the summed device time per kernel class and launches_host[MC_NKERNELS]
- * with the launch counts, pairs_host[MC_NKERNELS] with the pair evaluations (counted towards
- * N(N-1): rows x columns, no speculative work) each class covered.  Synchronises. */
-#define MC_K_TRIAL 0
-#define MC_K_BULK 1   /* rows of a chunk x columns outside chunks c-1, c                  */
-#define MC_K_FIX 2    /* rows of a chunk x columns of chunk c-1 (same kernel as MC_K_BULK) */
-#define MC_K_DIAG 3   /* rows of a chunk x columns of the chunk, with speculation          */
-#define MC_K_CHAIN 4  /* sequential resolution                                             */
-#define MC_NKERNELS 5
+ * does: same kernels, same arguments, bit-identical result) with CUDA events on the handle's stream
+ * around each of its two launches.  Fills ms_host[MC_NKERNELS] with the device time per kernel,
+ * launches_host[MC_NKERNELS] with the launch counts and pairs_host[MC_NKERNELS] with the pair
+ * evaluations that count towards N(N-1) (no speculative or correction work).  Synchronises. */
+#define MC_K_TRIAL 0  /* k_trial: a1                                          */
+#define MC_K_SWEEP 1  /* k_sweep: a2-a4, the whole sweep in one cooperative launch */
+#define MC_NKERNELS 2
 int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_t* pairs_host);
 
 /* Diagnostics of the persistent sweep kernel (option "debug" = 1): SM-clock cycle counters of the
@@ -143,19 +155,34 @@ int mc_debug_counters(mc_handle* h, int64_t* out16_host);
  * exactly once per chunk.  out4_host = {items, violations, widest item in columns, urgent items}. */
 int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers, int64_t* out4_host);
 
-/* Diagnostics: copies the first n ints of the persistent kernel's scheduling state (ticket
- * counters, progress counter, per-chunk completion counters) to the host on a stream of its own,
- * without waiting for the handle's stream (usable while a sweep is running). */
+/* Diagnostics: copies the first n ints of the sweep kernel's scheduling state (ticket counters,
+ * progress counter, per-chunk completion counters; n <= 256 + 4 (N / 256 + 1)) -- or, for n < 0, the
+ * first -n 32-bit words of the diagnostic counters (-n <= 2080) -- to the host on a stream of its
+ * own, without waiting for the handle's stream (usable while a sweep is running). */
 int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
 
-/* Tuning knobs (diagnostic; defaults are right for B200): key "chunk" = rows resolved per
- * chain kernel (multiple of 32, 32..1024), "graph" = 0/1 use CUDA graphs, "overlap" = 0/1 run
- * the chain concurrently with the next chunk's bulk kernel, "bulk_rows" = 1|2 rows per thread of
- * the bulk kernel, "bulk_ctas" = 1..4 bulk CTAs per SM the grid is sized for, "uniform_path" =
- * 0/1 allow the equal-diameter specialisation.  Every setting gives the same accept/reject
- * sequence; settings that change the partition of a row's sum change dE by rounding only.
- * Returns MC_EINVAL for unknown keys. */
+/* Options.  Every setting gives the same accept/reject sequence as the oracle; settings that change
+ * the partition of a row's sum change dE by rounding only (the sums themselves do not depend on the
+ * schedule).  Unknown keys and out-of-range values return MC_EINVAL.
+ *   "prows"        1|2|4   rows per thread of the sweep kernel; chunk = 256 * prows rows
+ *                          (default by N: 4 from 16384, 2 from 2048, else 1)
+ *   "far_cols"     8..65536, multiple of 8: target columns per FAR item (default 256)
+ *   "pnear"        0..128  worker CTAs that serve only urgent and in-chunk items (default 4)
+ *   "wave"         0|1     round a chunk's FAR items to a multiple of the FAR workers (default 1)
+ *   "form"         -1|0|1|2  pair-distance form (persist.cuh): -1 = by geometry (default): 0 GRAM if
+ *                          cavity_R / d_min <= 64, else 1 DIFFW if max_disp / d_min <= 64, else 2 CANON;
+ *                          a value below the automatic one is refused (it would break the dE bar)
+ *   "uniform_path" 0|1     allow the equal-diameter specialisation (default 1)
+ *   "stall_ms"     0..3600000  watchdog limit per wait of the sweep kernel in ms (default 2000; 0 = none;
+ *                          raise it under a profiler, a sanitizer or GPU time-slicing)
+ *   "hist_slices"  1..64   column slices of the pair-histogram kernel (default 32)
+ *   "debug"        0|1     collect the counters of mc_debug_counters (default 0)
+ *   "probe"        0|1|2   needs debug = 1.  1: the next sweeps run the worker loop alone over all columns
+ *                          (throughput probe); their results are meaningless and the sweep index stands still.
+ *                          2: the deciding warp never runs, so the next sweep stalls (tests MC_ESTALL)
+ * mc_get_option reads a setting back ("form_auto": the form the geometry allows). */
 int mc_set_option(mc_handle* h, const char* key, int64_t value);
+int mc_get_option(mc_handle* h, const char* key, int64_t* value_host);
 
 /* Number of kernels this handle launched (or replayed through graphs) since mc_init. */
 int mc_get_launch_count(mc_handle* h, uint64_t* n_host);

@@ -21,8 +21,9 @@ _CODES = {-1: "MC_EINVAL", -2: "MC_EOVERLAP", -3: "MC_EOUTSIDE", -4: "MC_ENOSPAC
 EXPORTS = (
     "mc_workspace_bytes", "mc_init", "mc_sweep", "mc_energy", "mc_energy_dev", "mc_pair_hist", "mc_sweep_host",
     "mc_sweep_timed",
-    "mc_get_positions", "mc_set_positions", "mc_get_sweep_index", "mc_set_sweep_index", "mc_get_stats",
-    "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option", "mc_debug_counters", "mc_debug_peek", "mc_plan_check",
+    "mc_get_positions", "mc_set_positions", "mc_set_state", "mc_get_sweep_index", "mc_set_sweep_index", "mc_get_stats",
+    "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option", "mc_get_option",
+    "mc_debug_counters", "mc_debug_peek", "mc_plan_check",
     "mc_get_launch_count",
 )
 
@@ -58,9 +59,10 @@ def load_library() -> C.CDLL:
     lib.mc_energy_dev.argtypes = [vp, vp]
     lib.mc_sweep_timed.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64), C.POINTER(i64)]
     lib.mc_pair_hist.argtypes = [vp, dbl, C.c_int, dbl, vp, vp]
-    lib.mc_sweep_host.argtypes = [vp, i64, vp, vp, C.POINTER(mc_stats)]
+    lib.mc_sweep_host.argtypes = [vp, i64, vp, C.POINTER(dbl), vp, C.POINTER(mc_stats)]
     lib.mc_get_positions.argtypes = [vp, vp]
     lib.mc_set_positions.argtypes = [vp, vp]
+    lib.mc_set_state.argtypes = [vp, vp, u64, dbl]
     lib.mc_get_sweep_index.argtypes = [vp, C.POINTER(u64)]
     lib.mc_set_sweep_index.argtypes = [vp, u64]
     lib.mc_get_stats.argtypes = [vp, C.POINTER(mc_stats)]
@@ -69,6 +71,7 @@ def load_library() -> C.CDLL:
     lib.mc_last_error.argtypes = []; lib.mc_last_error.restype = C.c_char_p
     lib.mc_measure_fp64_peak.argtypes = [vp, dbl, C.POINTER(dbl)]
     lib.mc_set_option.argtypes = [vp, C.c_char_p, i64]
+    lib.mc_get_option.argtypes = [vp, C.c_char_p, C.POINTER(i64)]
     lib.mc_get_launch_count.argtypes = [vp, C.POINTER(u64)]
     lib.mc_debug_counters.argtypes = [vp, C.POINTER(C.c_int64)]
     lib.mc_debug_peek.argtypes = [vp, C.POINTER(C.c_int32), C.c_int]
@@ -173,7 +176,7 @@ class MCSystem:
         _check(self._lib.mc_energy_dev(self._h, out.data_ptr()))
         return out
 
-    KERNEL_CLASSES = ("k_trial", "k_bulk", "k_bulk(fix)", "k_diag", "k_chain")
+    KERNEL_CLASSES = ("k_trial", "k_sweep")
 
     def mc_sweep_timed(self) -> dict:
         """One sweep with an event pair around every launch: {class: (ms, launches, pair evals)}."""
@@ -195,8 +198,9 @@ class MCSystem:
 
     pair_hist = mc_pair_hist
 
-    def mc_sweep_host(self, n, pos_in=None, pos_out=None):
-        """n sweeps through pinned host tensors; returns (pos_out, stats dict)."""
+    def mc_sweep_host(self, n, pos_in=None, pos_out=None, E_running_in=None):
+        """n sweeps through pinned host tensors; returns (pos_out, stats dict).  ``E_running_in``: the running
+        energy that belongs to ``pos_in`` (taken on trust: no from-scratch pass), or None to recompute it."""
         st = mc_stats()
         if pos_in is not None:
             assert not pos_in.is_cuda and pos_in.dtype == torch.float64 and pos_in.is_contiguous()
@@ -204,7 +208,8 @@ class MCSystem:
         if pos_out is not None:
             assert not pos_out.is_cuda and pos_out.dtype == torch.float64 and pos_out.is_contiguous()
             assert tuple(pos_out.shape) == (3, self.N)
-        _check(self._lib.mc_sweep_host(self._h, int(n), pos_in.data_ptr() if pos_in is not None else None,
+        e_in = C.byref(C.c_double(float(E_running_in))) if E_running_in is not None else None
+        _check(self._lib.mc_sweep_host(self._h, int(n), pos_in.data_ptr() if pos_in is not None else None, e_in,
                                        pos_out.data_ptr() if pos_out is not None else None, C.byref(st)))
         return pos_out, _stats_dict(st)
 
@@ -218,6 +223,11 @@ class MCSystem:
         p = _dev_f64(pos, (3, self.N), self.device)
         _check(self._lib.mc_set_positions(self._h, p.data_ptr()))
         self._keep = p  # keep alive until the stream has consumed it
+
+    def mc_set_state(self, pos, sweep_index: int, E_running: float):
+        p = _dev_f64(pos, (3, self.N), self.device)
+        _check(self._lib.mc_set_state(self._h, p.data_ptr(), int(sweep_index), float(E_running)))
+        self._keep = p
 
     @property
     def positions(self) -> np.ndarray:
@@ -254,6 +264,11 @@ class MCSystem:
 
     def mc_set_option(self, key: str, value: int):
         _check(self._lib.mc_set_option(self._h, key.encode(), int(value)))
+
+    def mc_get_option(self, key: str) -> int:
+        v = C.c_int64()
+        _check(self._lib.mc_get_option(self._h, key.encode(), C.byref(v)))
+        return v.value
 
     def mc_debug_counters(self) -> list:
         out = (C.c_int64 * 16)()

@@ -1,5 +1,6 @@
 // mcb200.cu -- host side of libmcb200.so: the C ABI declared in include/mcb200.h.
-// Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -fmad=false -shared -Xcompiler -fPIC
+// Build: paper_1602_05716_b200/build.py (nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -fmad=false; this file plus
+// sweep_inst.cu once per pair-distance form, linked into one shared object)
 #include "../../include/mcb200.h"
 
 #include <algorithm>
@@ -9,8 +10,8 @@
 #include <string>
 #include <vector>
 
-#include "kernels.cuh"
-#include "persist.cuh"
+#include "aux_kernels.cuh"
+#include "sweep_launch.h"
 
 using namespace mcb;
 
@@ -31,10 +32,11 @@ int fail(int code, const std::string& msg) {
     } while (0)
 
 constexpr size_t kAlign = 256;
+constexpr size_t kDbgWords = 16 + 1024;   // diagnostic counters of the sweep kernel (mc_debug_counters)
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t xy, zq, hh, lbq, txy, tz, lnu, wall, partA, ovA, partD, ovD, Dblk, OVold, OVnew, log_dE, log_flags,
+    size_t xy, zq, hh, lbq, txy, tz, lnu, wall, Dblk, OVold, OVnew, log_dE, log_flags,
         st, epart, centres, ccount, stage_pos, S1, S2, ovc, nn, sy, dbg, hcode, hcount, hcursor, hsxy, hszq, hbbox, total;
 };
 
@@ -48,16 +50,12 @@ Layout make_layout(int64_t N) {
     const size_t nt = kChunkMax / kTile;
     L.xy = take(Np * 16); L.zq = take(Np * 16); L.hh = take(Np * 8); L.lbq = take(Np * 8);
     L.txy = take(Np * 16); L.tz = take(Np * 8); L.lnu = take(Np * 8); L.wall = take(Np);
-    L.partA = take((size_t)2 * kMaxSlices * kChunkMax * 8); L.ovA = take((size_t)2 * kMaxSlices * kChunkMax * 4);
-    // double-buffered by chunk parity (the persistent kernel prepares chunk c+1 while the chain is in c)
-    L.partD = take(2 * nt * kChunkMax * 8); L.ovD = take(2 * nt * kChunkMax * 4);
+    // double-buffered by chunk parity (the sweep kernel prepares chunk c+1 while the chain is in c)
     L.Dblk = take(2 * (nt * (nt + 1) / 2) * kTile * kTile * 8);
     L.OVold = take((size_t)2 * kChunkMax * nt * 4); L.OVnew = take((size_t)2 * kChunkMax * nt * 4);
     L.S1 = take(Np * 8); L.S2 = take(Np * 8); L.ovc = take(Np * 4); L.nn = take(Np * 8);
-    take(65536);
     L.sy = take((size_t)(kSyHdr + 4 * (Np / 256 + 1)) * 4);
-    take(65536);
-    L.dbg = take(16 * 8 + 1024 * 8);
+    L.dbg = take(kDbgWords * 8);
     L.hcode = take(Np * 4); L.hcount = take((size_t)kCells * 4); L.hcursor = take((size_t)kCells * 4);
     L.hsxy = take(Np * 16); L.hszq = take(Np * 16); L.hbbox = take((Np / 256 + 1) * 4 * 6 * 8);
     L.log_dE = take(Np * 8); L.log_flags = take(Np);
@@ -71,35 +69,28 @@ Layout make_layout(int64_t N) {
 
 }  // namespace
 
+
 struct mc_handle {
     Params p{};
     Layout L{};
     char* ws = nullptr;
     cudaStream_t stream = nullptr;
-    cudaStream_t cap_stream = nullptr;   // graph capture origin (bulk kernels)
-    cudaStream_t cap_stream2 = nullptr;  // chain branch of the captured graph
-    cudaEvent_t ev_trial = nullptr, ev_bulk[2] = {nullptr, nullptr}, ev_chain[2] = {nullptr, nullptr};
     int num_sms = 148;
-    int chunk = kChunkMax;
-    bool use_graph = true;
-    bool overlap = true;
-    int engine = 1;          // 1: one persistent kernel per sweep (persist.cuh); 0: kernels per chunk in a graph
-    int prows = 4;           // rows per consumer thread of the persistent kernel (chunk = 256 * prows)
-    int pfarcols = 256;      // columns per FAR item of the persistent kernel
+    int prows = 4;           // rows per consumer thread of the sweep kernel (chunk = 256 * prows)
+    int pfarcols = 256;      // columns per FAR item of the sweep kernel
     int hist_slices = kHistSlices;   // column slices (grid.y) of k_hist
-    int pmode = 0;           // 1: throughput probe (diagnostic; the sweep's results are meaningless)
+    int pmode = 0;           // 1: throughput probe (diagnostic, needs "debug"; the sweep's results are meaningless)
     bool pwave = true;       // round the FAR items of a chunk to a multiple of the FAR workers
-    int pnear = 4;           // worker CTAs of the persistent kernel that serve FIX and DIAG items only
+    int pnear = 4;           // worker CTAs of the sweep kernel that serve urgent and DIAG items only
     bool debug = false;      // collect the cycle counters of mc_debug_counters
-    int pgrid = 0;           // CTAs of the persistent kernel (0: not yet configured)
-    int bulk_rows = 1;       // rows per consumer thread of k_bulk (1 or 2)
-    int bulk_ctas = 2;       // k_bulk CTAs per SM the grid is sized for
+    int pgrid = 0;           // CTAs of the sweep kernel
+    int pgrid_key = -1;      // (form, rows, uniform) the grid was sized and the kernel configured for
     bool uniform_d = false;  // all diameters equal: s_ij^2 is one constant
     bool allow_uniform = true;
     bool all_d_equal = false;
-    cudaGraphExec_t graph = nullptr;
+    int form_auto = kFormGram;   // pair-distance form the geometry allows (mc_init)
+    int form = kFormGram;        // form in use (option "form": the automatic one or a more exact one)
     uint64_t launches = 0;
-    uint64_t launches_per_sweep = 0;
     double* epart = nullptr;
     int* centres = nullptr;
     int* ccount = nullptr;
@@ -108,151 +99,29 @@ struct mc_handle {
 
 namespace {
 
-void drop_graph(mc_handle* h) {
-    if (h->graph) {
-        cudaGraphExecDestroy(h->graph);
-        h->graph = nullptr;
-    }
-}
+// geometry limits of the pair-distance forms (persist.cuh)
+constexpr double kGramMaxRatio = 64.0;    // GRAM  needs cavity_R / d_min <= 64
+constexpr double kDiffWMaxRatio = 64.0;   // DIFFW needs max_disp / d_min <= 64
 
-int bulk_row_groups(const mc_handle* h, int nrows) {
-    const int per = kBulkThreads * h->bulk_rows;
-    return (nrows + per - 1) / per;
-}
-
-int slices_for(const mc_handle* h, int nrows, int ncols) {
-    const int rgs = bulk_row_groups(h, nrows);
-    // bulk_ctas CTAs per SM on all SMs but one: the chain CTA of the previous chunk (which runs
-    // concurrently on the other graph branch) needs a whole SM's registers
-    int target = (h->bulk_ctas * (h->num_sms - 1)) / rgs;
-    const int max_by_cols = ncols / 64 > 0 ? ncols / 64 : 1;  // at least 64 columns per slice
-    if (target > max_by_cols) target = max_by_cols;
-    if (target > kMaxSlices - 64) target = kMaxSlices - 64;
-    if (target < 1) target = 1;
-    return target;
-}
-
-void launch_bulk(const mc_handle* h, cudaStream_t s, const Params& pc, int row0, int nrows, int cbeg, int cend,
-                 int gap0, int gap1, int nsl, int slot0) {
-    const dim3 grid(bulk_row_groups(h, nrows), nsl), block(kBulkThreads + 32);
-    if (h->bulk_rows == 2) {
-        if (h->uniform_d) k_bulk<2, true><<<grid, block, 0, s>>>(pc, row0, nrows, cbeg, cend, gap0, gap1, nsl, slot0);
-        else k_bulk<2, false><<<grid, block, 0, s>>>(pc, row0, nrows, cbeg, cend, gap0, gap1, nsl, slot0);
-    } else {
-        if (h->uniform_d) k_bulk<1, true><<<grid, block, 0, s>>>(pc, row0, nrows, cbeg, cend, gap0, gap1, nsl, slot0);
-        else k_bulk<1, false><<<grid, block, 0, s>>>(pc, row0, nrows, cbeg, cend, gap0, gap1, nsl, slot0);
-    }
-}
-
-// Optional per-launch timing (mc_sweep_timed): an event pair around every launch, serial mode only.
-struct SweepTimer {
-    std::vector<cudaEvent_t> ev;   // 2 per launch
-    std::vector<int> kind;
-    int64_t pairs[MC_NKERNELS] = {0, 0, 0, 0, 0};
-    void before(cudaStream_t s, int k) {
-        cudaEvent_t a, b;
-        cudaEventCreate(&a); cudaEventCreate(&b);
-        ev.push_back(a); ev.push_back(b); kind.push_back(k);
-        cudaEventRecord(a, s);
-    }
-    void after(cudaStream_t s) { cudaEventRecord(ev.back(), s); }
-};
-
-// Enqueue one sweep.  sa carries k_trial and the bulk kernels, sb the per-chunk fix/diag/chain
-// kernels.  With sb == sa everything is serial; with two capturing streams (fork = true) the
-// chain of chunk c runs concurrently with the bulk kernel of chunk c+1:
-//   bulk(c)  : rows of chunk c x columns outside chunks c-1 and c      needs chain(c-2)
-//   fix(c)   : rows of chunk c x columns of chunk c-1 (final)          needs chain(c-1)
-//   diag(c)  : rows of chunk c x columns of chunk c                    needs chain(c-1) (buffers)
-//   chain(c) : needs bulk(c), fix(c), diag(c)
-// Both modes launch the same kernels with the same arguments, so results are bit-identical.
-int enqueue_sweep(mc_handle* h, cudaStream_t sa, cudaStream_t sb, bool fork, uint64_t* count,
-                  SweepTimer* tm = nullptr) {
-    Params p = h->p;
-    p.chunk = h->chunk;
-    uint64_t n = 0;
-    if (tm) tm->before(sa, MC_K_TRIAL);
-    k_trial<<<(p.Np + 255) / 256, 256, 0, sa>>>(p);
-    if (tm) tm->after(sa);
-    ++n;
-    if (fork) {
-        cudaEventRecord(h->ev_trial, sa);
-        cudaStreamWaitEvent(sb, h->ev_trial, 0);
-    }
-    const int nchunks = (p.Np + h->chunk - 1) / h->chunk;
-    for (int c = 0; c < nchunks; ++c) {
-        const int row0 = c * h->chunk;
-        const int nrows = std::min(h->chunk, p.Np - row0);
-        const int prev0 = c > 0 ? row0 - h->chunk : row0;   // start of chunk c-1 (== row0 for c == 0)
-        const int ncols = p.Np - (row0 + nrows - prev0);
-        const int64_t real_rows = std::max(0, std::min(nrows, p.N - row0));
-        Params pc = p;   // partial buffers alternate with the chunk parity
-        pc.partA = p.partA + (size_t)(c & 1) * kMaxSlices * kChunkMax;
-        pc.ovA = p.ovA + (size_t)(c & 1) * kMaxSlices * kChunkMax;
-        int nslA = 0, nslF = 0;
-        if (fork && c >= 2) cudaStreamWaitEvent(sa, h->ev_chain[c & 1], 0);
-        if (ncols > 0) {
-            nslA = slices_for(h, nrows, ncols);
-            if (tm) {
-                tm->before(sa, MC_K_BULK);
-                tm->pairs[MC_K_BULK] += real_rows * (int64_t)(p.N - std::min(p.N, row0 + nrows) + prev0);
-            }
-            launch_bulk(h, sa, pc, row0, nrows, 0, p.Np, prev0, row0 + nrows, nslA, 0);
-            if (tm) tm->after(sa);
-            ++n;
-        }
-        if (fork) cudaEventRecord(h->ev_bulk[c & 1], sa);
-        if (c > 0) {
-            nslF = std::max(1, std::min(32, (row0 - prev0) / 32));
-            if (tm) {
-                tm->before(sb, MC_K_FIX);
-                tm->pairs[MC_K_FIX] += real_rows * (int64_t)(row0 - prev0);
-            }
-            launch_bulk(h, sb, pc, row0, nrows, prev0, row0, row0, row0, nslF, nslA);
-            if (tm) tm->after(sb);
-            ++n;
-        }
-        const int nt = nrows / kTile;
-        if (tm) {
-            tm->before(sb, MC_K_DIAG);
-            tm->pairs[MC_K_DIAG] += real_rows * (real_rows - 1);
-        }
-        k_diag<<<(nt * nt + 7) / 8, 256, 0, sb>>>(pc, row0, nrows);
-        if (tm) tm->after(sb);
-        ++n;
-        if (fork) cudaStreamWaitEvent(sb, h->ev_bulk[c & 1], 0);
-        if (tm) tm->before(sb, MC_K_CHAIN);
-        k_chain<<<1, kChainThreads, 0, sb>>>(pc, row0, nrows, nslA + nslF, c == nchunks - 1 ? 1 : 0);
-        if (tm) tm->after(sb);
-        ++n;
-        if (fork) cudaEventRecord(h->ev_chain[c & 1], sb);
-    }
-    if (fork) cudaStreamWaitEvent(sa, h->ev_chain[(nchunks - 1) & 1], 0);   // join
-    if (count) *count = n;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return fail(MC_ECUDA, std::string("sweep launch: ") + cudaGetErrorString(e));
-    return MC_OK;
-}
-
-// ---- persistent engine (persist.cuh): k_trial + one cooperative k_sweep launch per sweep ----
-template <int ROWS, bool UNIFORM>
-int launch_sweep_kernel(mc_handle* h, cudaStream_t s) {
-    auto kern = k_sweep<ROWS, UNIFORM>;
-    const int smem = (int)sizeof(PShared);
-    static thread_local bool configured = false;
-    if (!configured) {
-        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        configured = true;
-    }
-    if (h->pgrid == 0) {
+int launch_sweep(mc_handle* h, cudaStream_t s) {
+    SweepLaunch L{};
+    L.rows = h->prows;
+    L.uniform = h->uniform_d;
+    L.stream = s;
+    auto fn = h->form == kFormGram ? launch_sweep_gram : h->form == kFormDiffW ? launch_sweep_diffw : launch_sweep_canon;
+    const int key = h->form * 16 + h->prows * 2 + (h->uniform_d ? 1 : 0);
+    if (h->pgrid_key != key) {
         int occ = 0;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kPThreads, smem));
+        L.grid = 0;
+        const cudaError_t e = (cudaError_t)fn(L, &occ);
+        if (e != cudaSuccess) return fail(MC_ECUDA, std::string("k_sweep configuration: ") + cudaGetErrorString(e));
         if (occ < 1) return fail(MC_ECUDA, "k_sweep does not fit on an SM");
         h->pgrid = std::min(occ, 2) * h->num_sms;
+        h->pgrid_key = key;
     }
-    PArgs a{};
+    PArgs& a = L.args;
     a.p = h->p;
-    a.C = 256 * ROWS;
+    a.C = 256 * h->prows;
     a.p.chunk = a.C;
     a.nchunks = (a.p.Np + a.C - 1) / a.C;
     a.nnear = std::min(h->pnear, std::max(0, h->pgrid - 4));
@@ -260,64 +129,44 @@ int launch_sweep_kernel(mc_handle* h, cudaStream_t s) {
     a.mode = h->pmode;
     a.nfar = h->pwave ? std::max(1, h->pgrid - 2 - a.nnear) : 0;
     a.sy = h->p.sy;
-    char* w = h->ws;
-    a.dbg = h->debug ? (long long*)(w + h->L.dbg) : nullptr;
-    if (a.dbg) CUDA_TRY(cudaMemsetAsync(a.dbg, 0, 16 * 8 + 1024 * 8, s));
-    void* args[] = {(void*)&a};
-    CUDA_TRY(cudaLaunchCooperativeKernel((void*)kern, dim3(h->pgrid), dim3(kPThreads), args, (size_t)smem, s));
+    a.dbg = h->debug ? (long long*)(h->ws + h->L.dbg) : nullptr;
+    if (a.dbg) CUDA_TRY(cudaMemsetAsync(a.dbg, 0, kDbgWords * 8, s));
+    L.grid = h->pgrid;
+    const cudaError_t e = (cudaError_t)fn(L, nullptr);
+    if (e != cudaSuccess) return fail(MC_ECUDA, std::string("k_sweep launch: ") + cudaGetErrorString(e));
     return MC_OK;
 }
 
-int enqueue_sweep_persist(mc_handle* h, cudaStream_t s) {
+// one sweep: k_trial (a1; also resets the scheduling words and the row accumulators), then k_sweep (a2-a4)
+int enqueue_sweep(mc_handle* h, cudaStream_t s) {
     const Params& p = h->p;
     k_trial<<<(p.Np + 255) / 256, 256, 0, s>>>(p);
     CUDA_TRY(cudaGetLastError());
-    const bool u = h->uniform_d;
-    switch (h->prows) {
-        case 1: return u ? launch_sweep_kernel<1, true>(h, s) : launch_sweep_kernel<1, false>(h, s);
-        case 2: return u ? launch_sweep_kernel<2, true>(h, s) : launch_sweep_kernel<2, false>(h, s);
-        default: return u ? launch_sweep_kernel<4, true>(h, s) : launch_sweep_kernel<4, false>(h, s);
-    }
-}
-
-int build_graph(mc_handle* h) {
-    drop_graph(h);
-    cudaGraph_t g = nullptr;
-    // capture on private streams (the caller's may be the legacy default stream, which cannot capture)
-    if (!h->cap_stream) {
-        CUDA_TRY(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
-        CUDA_TRY(cudaStreamCreateWithFlags(&h->cap_stream2, cudaStreamNonBlocking));
-        CUDA_TRY(cudaEventCreateWithFlags(&h->ev_trial, cudaEventDisableTiming));
-        for (int k = 0; k < 2; ++k) {
-            CUDA_TRY(cudaEventCreateWithFlags(&h->ev_bulk[k], cudaEventDisableTiming));
-            CUDA_TRY(cudaEventCreateWithFlags(&h->ev_chain[k], cudaEventDisableTiming));
-        }
-    }
-    CUDA_TRY(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
-    uint64_t n = 0;
-    const int rc = h->overlap ? enqueue_sweep(h, h->cap_stream, h->cap_stream2, true, &n)
-                              : enqueue_sweep(h, h->cap_stream, h->cap_stream, false, &n);
-    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
-    if (rc != MC_OK) {
-        if (g) cudaGraphDestroy(g);
-        return rc;
-    }
-    if (e != cudaSuccess) return fail(MC_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
-    e = cudaGraphInstantiate(&h->graph, g, 0);
-    cudaGraphDestroy(g);
-    if (e != cudaSuccess) return fail(MC_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e));
-    h->launches_per_sweep = n;
-    return MC_OK;
+    return launch_sweep(h, s);
 }
 
 int enqueue_energy(mc_handle* h, double* out_dev, int set_running, int check_overlap) {
     const Params& p = h->p;
     const int units = energy_units(p.Np);
-    if (check_overlap) k_energy<true><<<units, 256, 0, h->stream>>>(p, h->epart);
-    else k_energy<false><<<units, 256, 0, h->stream>>>(p, h->epart);
+    const bool gram = h->form_auto == kFormGram;
+    if (check_overlap) k_energy<true, false><<<units, 256, 0, h->stream>>>(p, h->epart);
+    else if (gram) k_energy<false, true><<<units, 256, 0, h->stream>>>(p, h->epart);
+    else k_energy<false, false><<<units, 256, 0, h->stream>>>(p, h->epart);
     k_energy_reduce<<<1, 32, 0, h->stream>>>(p, h->epart, units, out_dev, set_running);
     h->launches += 2;
     CUDA_TRY(cudaGetLastError());
+    return MC_OK;
+}
+
+// Waits for the handle's stream and reports a stalled sweep (the watchdog of persist.cuh): after
+// MC_ESTALL the configuration is invalid until mc_set_positions / mc_set_state replaces it.
+int sync_and_check(mc_handle* h) {
+    int stall = 0;
+    CUDA_TRY(cudaMemcpyAsync(&stall, &h->p.st->stall, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    if (stall)
+        return fail(MC_ESTALL, "a sweep stalled (a wait of the sweep kernel exceeded stall_ms); the state is invalid "
+                               "until mc_set_positions or mc_set_state replaces it");
     return MC_OK;
 }
 
@@ -342,6 +191,7 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     if (!(cavity_R > 0) || !(bjerrum_length >= 0) || !(max_disp >= 0) || !std::isfinite(cavity_R) ||
         !std::isfinite(bjerrum_length) || !std::isfinite(max_disp))
         return fail(MC_EINVAL, "cavity_R must be > 0, bjerrum_length >= 0, max_disp >= 0, all finite");
+    if (cavity_R > 1.0e7) return fail(MC_EINVAL, "cavity_R must not exceed 1e7 (padding particles are parked at 1e9)");
     if (((uintptr_t)workspace_dev % kAlign) != 0) return fail(MC_EINVAL, "workspace must be 256-byte aligned");
     const Layout L = make_layout(N);
     if (workspace_bytes < L.total) return fail(MC_ENOSPACE, "workspace smaller than mc_workspace_bytes(N)");
@@ -359,13 +209,11 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     h->stream = (cudaStream_t)stream;
     h->num_sms = prop.multiProcessorCount;
     Params& p = h->p;
-    p.N = (int)N; p.Np = padded(N); p.chunk = h->chunk;
+    p.N = (int)N; p.Np = padded(N); p.chunk = kChunkMax;
     char* w = h->ws;
     p.xy = (double2*)(w + L.xy); p.zq = (double2*)(w + L.zq); p.hh = (double*)(w + L.hh);
     p.lbq = (double*)(w + L.lbq); p.txy = (double2*)(w + L.txy); p.tz = (double*)(w + L.tz);
     p.lnu = (double*)(w + L.lnu); p.wall = (unsigned char*)(w + L.wall);
-    p.partA = (double*)(w + L.partA); p.ovA = (int*)(w + L.ovA);
-    p.partD = (double*)(w + L.partD); p.ovD = (int*)(w + L.ovD);
     p.Dblk = (double*)(w + L.Dblk); p.OVold = (unsigned*)(w + L.OVold); p.OVnew = (unsigned*)(w + L.OVnew);
     p.log_dE = (double*)(w + L.log_dE); p.log_flags = (unsigned char*)(w + L.log_flags);
     p.st = (DevState*)(w + L.st);
@@ -375,6 +223,7 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     p.sy_n = kSyHdr + 4 * (p.Np / 256 + 1);   // header + per-chunk counters
     h->prows = p.Np >= 16384 ? 4 : (p.Np >= 2048 ? 2 : 1);
     p.R = cavity_R; p.lB = bjerrum_length; p.max_disp = max_disp; p.seed = seed;
+    p.wait_limit_ns = 2000000000ull;
     h->epart = (double*)(w + L.epart);
     h->centres = (int*)(w + L.centres);
     h->ccount = (int*)(w + L.ccount);
@@ -393,7 +242,7 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     k_check_particles<<<nb, 256, 0, h->stream>>>(p, diameters_dev);
     h->launches += 2;
     if (validate) {
-        const int rc = enqueue_energy(h, nullptr, 1, 1);
+        const int rc = enqueue_energy(h, nullptr, 1, 1);   // exact differences: no geometry assumption yet
         if (rc != MC_OK) return bail(rc);
     }
     DevState st{};
@@ -401,20 +250,20 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return bail(fail(MC_ECUDA, std::string("init: ") + cudaGetErrorString(e)));
     h->all_d_equal = st.d_differs == 0;
-    if (st.err == 0) {
-        // the sweep kernels form r^2 from |x_i|^2 + |x_j|^2 - 2 x_i.x_j and re-examine a veto exactly only
-        // within 2^-16 relative of the contact distance: that needs (R / d_min)^2 * 2^-50 << 2^-16
-        double dmin;
-        std::memcpy(&dmin, &st.dmin_bits, sizeof(dmin));
-        if (!(dmin > 0) || cavity_R / dmin > 2.0e4)
-            return bail(fail(MC_EINVAL, "cavity_R / smallest diameter exceeds 2e4: outside the range the FP64 veto band covers"));
-    }
     h->uniform_d = h->allow_uniform && h->all_d_equal;
     if (st.err != 0) {
         if (st.err <= -1000) return bail(fail(MC_EINVAL, "non-finite input or diameter <= 0"));
         if (st.err == -3) return bail(fail(MC_EOUTSIDE, "an ion sticks out of the cavity"));
         return bail(fail(MC_EOVERLAP, "two ions overlap in the initial configuration"));
     }
+    double dmin;
+    std::memcpy(&dmin, &st.dmin_bits, sizeof(dmin));
+    if (!(dmin > 0) || cavity_R / dmin > 1.0e6)
+        return bail(fail(MC_EINVAL, "cavity_R / smallest diameter exceeds 1e6: FP64 positions no longer resolve 1e-10 d"));
+    // pair-distance form by geometry (persist.cuh): the cheapest one whose error stays inside the dE bar
+    h->form_auto = cavity_R / dmin <= kGramMaxRatio ? kFormGram : max_disp / dmin <= kDiffWMaxRatio ? kFormDiffW : kFormCanon;
+    h->form = h->form_auto;
+    p.ov_tol = 0x1.0p-20 * dmin * dmin;
     *out = h;
     return MC_OK;
 }
@@ -422,43 +271,17 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
 int mc_free(mc_handle* h) {
     if (!h) return MC_OK;
     cudaStreamSynchronize(h->stream);
-    drop_graph(h);
-    if (h->cap_stream) {
-        cudaStreamDestroy(h->cap_stream);
-        cudaStreamDestroy(h->cap_stream2);
-        cudaEventDestroy(h->ev_trial);
-        for (int k = 0; k < 2; ++k) { cudaEventDestroy(h->ev_bulk[k]); cudaEventDestroy(h->ev_chain[k]); }
-    }
     delete h;
     return MC_OK;
 }
 
 int mc_sweep(mc_handle* h, int64_t n) {
     if (!h || n < 0) return fail(MC_EINVAL, "bad handle or n < 0");
-    if (n == 0) return MC_OK;
-    if (h->engine == 1) {
-        for (int64_t s = 0; s < n; ++s) {
-            const int rc = enqueue_sweep_persist(h, h->stream);
-            if (rc != MC_OK) return rc;
-        }
-        h->launches += 2 * (uint64_t)n;
-        return MC_OK;
+    for (int64_t s = 0; s < n; ++s) {
+        const int rc = enqueue_sweep(h, h->stream);
+        if (rc != MC_OK) return rc;
     }
-    if (h->use_graph) {
-        if (!h->graph) {
-            const int rc = build_graph(h);
-            if (rc != MC_OK) return rc;
-        }
-        for (int64_t s = 0; s < n; ++s) CUDA_TRY(cudaGraphLaunch(h->graph, h->stream));
-        h->launches += h->launches_per_sweep * (uint64_t)n;
-    } else {
-        for (int64_t s = 0; s < n; ++s) {
-            uint64_t c = 0;
-            const int rc = enqueue_sweep(h, h->stream, h->stream, false, &c);
-            if (rc != MC_OK) return rc;
-            h->launches += c;
-        }
-    }
+    h->launches += 2 * (uint64_t)n;
     return MC_OK;
 }
 
@@ -468,8 +291,7 @@ int mc_energy(mc_handle* h, double* E_host) {
     const int rc = enqueue_energy(h, out, 0, 0);
     if (rc != MC_OK) return rc;
     CUDA_TRY(cudaMemcpyAsync(E_host, out, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
-    return MC_OK;
+    return sync_and_check(h);
 }
 
 int mc_energy_dev(mc_handle* h, double* E_dev) {
@@ -479,54 +301,27 @@ int mc_energy_dev(mc_handle* h, double* E_dev) {
 
 int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_t* pairs_host) {
     if (!h || !ms_host || !launches_host || !pairs_host) return fail(MC_EINVAL, "null argument");
-    if (h->engine == 1) {
-        // persistent engine: k_trial, then the whole sweep in one k_sweep launch (reported as MC_K_BULK)
-        for (int k = 0; k < MC_NKERNELS; ++k) { ms_host[k] = 0.0; launches_host[k] = 0; pairs_host[k] = 0; }
-        cudaEvent_t ev[3];
-        for (auto& x : ev) CUDA_TRY(cudaEventCreate(&x));
-        const Params& p = h->p;
-        // same launches as enqueue_sweep_persist, with an event between the two kernels
-        const int saved = h->engine;
-        (void)saved;
-        CUDA_TRY(cudaEventRecord(ev[0], h->stream));
-        k_trial<<<(p.Np + 255) / 256, 256, 0, h->stream>>>(p);
-        CUDA_TRY(cudaEventRecord(ev[1], h->stream));
-        const bool u = h->uniform_d;
-        int rc = MC_OK;
-        switch (h->prows) {
-            case 1: rc = u ? launch_sweep_kernel<1, true>(h, h->stream) : launch_sweep_kernel<1, false>(h, h->stream); break;
-            case 2: rc = u ? launch_sweep_kernel<2, true>(h, h->stream) : launch_sweep_kernel<2, false>(h, h->stream); break;
-            default: rc = u ? launch_sweep_kernel<4, true>(h, h->stream) : launch_sweep_kernel<4, false>(h, h->stream); break;
-        }
-        if (rc != MC_OK) return rc;
-        CUDA_TRY(cudaEventRecord(ev[2], h->stream));
-        CUDA_TRY(cudaStreamSynchronize(h->stream));
-        h->launches += 2;
-        float a = 0.f, b = 0.f;
-        CUDA_TRY(cudaEventElapsedTime(&a, ev[0], ev[1]));
-        CUDA_TRY(cudaEventElapsedTime(&b, ev[1], ev[2]));
-        for (auto& x : ev) cudaEventDestroy(x);
-        ms_host[MC_K_TRIAL] = a; launches_host[MC_K_TRIAL] = 1;
-        ms_host[MC_K_BULK] = b; launches_host[MC_K_BULK] = 1;
-        pairs_host[MC_K_BULK] = (int64_t)p.N * (int64_t)(p.N - 1);
-        return MC_OK;
-    }
-    SweepTimer tm;
-    uint64_t c = 0;
-    const int rc = enqueue_sweep(h, h->stream, h->stream, false, &c, &tm);
-    h->launches += c;
-    cudaError_t e = cudaStreamSynchronize(h->stream);
-    for (int k = 0; k < MC_NKERNELS; ++k) { ms_host[k] = 0.0; launches_host[k] = 0; pairs_host[k] = tm.pairs[k]; }
-    for (size_t i = 0; i < tm.kind.size(); ++i) {
-        float ms = 0.f;
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, tm.ev[2 * i], tm.ev[2 * i + 1]);
-        ms_host[tm.kind[i]] += ms;
-        launches_host[tm.kind[i]] += 1;
-    }
-    for (cudaEvent_t ev : tm.ev) cudaEventDestroy(ev);
+    for (int k = 0; k < MC_NKERNELS; ++k) { ms_host[k] = 0.0; launches_host[k] = 0; pairs_host[k] = 0; }
+    cudaEvent_t ev[3];
+    for (auto& x : ev) CUDA_TRY(cudaEventCreate(&x));
+    const Params& p = h->p;
+    // the launches of mc_sweep(h, 1), with an event between the two kernels
+    CUDA_TRY(cudaEventRecord(ev[0], h->stream));
+    k_trial<<<(p.Np + 255) / 256, 256, 0, h->stream>>>(p);
+    CUDA_TRY(cudaEventRecord(ev[1], h->stream));
+    const int rc = launch_sweep(h, h->stream);
     if (rc != MC_OK) return rc;
-    if (e != cudaSuccess) return fail(MC_ECUDA, std::string("mc_sweep_timed: ") + cudaGetErrorString(e));
-    return MC_OK;
+    CUDA_TRY(cudaEventRecord(ev[2], h->stream));
+    h->launches += 2;
+    const int rs = sync_and_check(h);
+    float a = 0.f, b = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&a, ev[0], ev[1]));
+    CUDA_TRY(cudaEventElapsedTime(&b, ev[1], ev[2]));
+    for (auto& x : ev) cudaEventDestroy(x);
+    ms_host[MC_K_TRIAL] = a; launches_host[MC_K_TRIAL] = 1;
+    ms_host[MC_K_SWEEP] = b; launches_host[MC_K_SWEEP] = 1;
+    pairs_host[MC_K_SWEEP] = (int64_t)p.N * (int64_t)(p.N - 1);
+    return rs;
 }
 
 int mc_pair_hist(mc_handle* h, double bin_width, int nbins, double centre_rmax, uint64_t* hist_dev,
@@ -584,18 +379,29 @@ int mc_get_positions(mc_handle* h, double* pos_dev_out) {
 int mc_set_positions(mc_handle* h, const double* pos_dev) {
     if (!h || !pos_dev) return fail(MC_EINVAL, "null argument");
     k_pack<<<(h->p.Np + 255) / 256, 256, 0, h->stream>>>(h->p, pos_dev, nullptr, nullptr);
-    h->launches += 1;
+    k_set_state<<<1, 1, 0, h->stream>>>(h->p.st, 0ull, 0, 0.0, 0);
+    h->launches += 2;
     CUDA_TRY(cudaGetLastError());
     return enqueue_energy(h, nullptr, 1, 0);
+}
+
+int mc_set_state(mc_handle* h, const double* pos_dev, uint64_t sweep_index, double E_running) {
+    if (!h || !pos_dev) return fail(MC_EINVAL, "null argument");
+    if (!std::isfinite(E_running)) return fail(MC_EINVAL, "E_running must be finite");
+    k_pack<<<(h->p.Np + 255) / 256, 256, 0, h->stream>>>(h->p, pos_dev, nullptr, nullptr);
+    k_set_state<<<1, 1, 0, h->stream>>>(h->p.st, (unsigned long long)sweep_index, 1, E_running, 1);
+    h->launches += 2;
+    CUDA_TRY(cudaGetLastError());
+    return MC_OK;
 }
 
 int mc_get_sweep_index(mc_handle* h, uint64_t* s_host) {
     if (!h || !s_host) return fail(MC_EINVAL, "null argument");
     unsigned long long s = 0;
     CUDA_TRY(cudaMemcpyAsync(&s, &h->p.st->sweep, sizeof(s), cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    const int rc = sync_and_check(h);
     *s_host = s;
-    return MC_OK;
+    return rc;
 }
 
 int mc_set_sweep_index(mc_handle* h, uint64_t s) {
@@ -614,7 +420,7 @@ int mc_get_stats(mc_handle* h, mc_stats* stats_host) {
     stats_host->accepted = st.accepted; stats_host->veto_overlap = st.veto_overlap;
     stats_host->veto_wall = st.veto_wall; stats_host->near_ties = st.near_ties;
     stats_host->E_running = st.E_run;
-    if (st.stall) return fail(MC_ESTALL, "the sweep kernel's watchdog fired: a wait exceeded its time limit");
+    if (st.stall) return sync_and_check(h);
     return MC_OK;
 }
 
@@ -626,13 +432,22 @@ int mc_get_trial_log(mc_handle* h, double* dE_dev, uint8_t* flags_dev) {
     return MC_OK;
 }
 
-int mc_sweep_host(mc_handle* h, int64_t n, const double* pos_in_host, double* pos_out_host,
-                  mc_stats* stats_host) {
+int mc_sweep_host(mc_handle* h, int64_t n, const double* pos_in_host, const double* E_running_in,
+                  double* pos_out_host, mc_stats* stats_host) {
     if (!h || n < 0) return fail(MC_EINVAL, "bad handle or n < 0");
     const size_t bytes = 3 * (size_t)h->p.N * sizeof(double);
     if (pos_in_host) {
         CUDA_TRY(cudaMemcpyAsync(h->stage_pos, pos_in_host, bytes, cudaMemcpyHostToDevice, h->stream));
-        const int rc = mc_set_positions(h, h->stage_pos);
+        int rc;
+        if (E_running_in) {   // the caller vouches for the running energy of this configuration: no O(N^2) pass
+            if (!std::isfinite(*E_running_in)) return fail(MC_EINVAL, "E_running_in must be finite");
+            k_pack<<<(h->p.Np + 255) / 256, 256, 0, h->stream>>>(h->p, h->stage_pos, nullptr, nullptr);
+            k_set_state<<<1, 1, 0, h->stream>>>(h->p.st, 0ull, 0, *E_running_in, 1);
+            h->launches += 2;
+            rc = cudaGetLastError() == cudaSuccess ? MC_OK : fail(MC_ECUDA, "mc_sweep_host: launch failed");
+        } else {
+            rc = mc_set_positions(h, h->stage_pos);
+        }
         if (rc != MC_OK) return rc;
     }
     int rc = mc_sweep(h, n);
@@ -643,8 +458,7 @@ int mc_sweep_host(mc_handle* h, int64_t n, const double* pos_in_host, double* po
         CUDA_TRY(cudaMemcpyAsync(pos_out_host, h->stage_pos, bytes, cudaMemcpyDeviceToHost, h->stream));
     }
     if (stats_host) return mc_get_stats(h, stats_host);
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
-    return MC_OK;
+    return sync_and_check(h);
 }
 
 int mc_measure_fp64_peak(void* stream, double millis, double* dfma_per_second_host) {
@@ -680,47 +494,59 @@ int mc_measure_fp64_peak(void* stream, double millis, double* dfma_per_second_ho
 
 int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     if (!h || !key) return fail(MC_EINVAL, "null argument");
-    if (!std::strcmp(key, "chunk")) {
-        if (value < kTile || value > kChunkMax || value % kTile) return fail(MC_EINVAL, "chunk must be a multiple of 32 in 32..1024");
-        h->chunk = (int)value;
-    } else if (!std::strcmp(key, "engine")) {
-        if (value != 0 && value != 1) return fail(MC_EINVAL, "engine must be 0 or 1");
-        h->engine = (int)value;
+    if (!std::strcmp(key, "prows")) {
+        if (value != 1 && value != 2 && value != 4) return fail(MC_EINVAL, "prows must be 1, 2 or 4");
+        h->prows = (int)value;
     } else if (!std::strcmp(key, "far_cols")) {
         if (value < 8 || value > 65536 || value % 8) return fail(MC_EINVAL, "far_cols must be a multiple of 8 in 8..65536");
         h->pfarcols = (int)value;
-    } else if (!std::strcmp(key, "hist_slices")) {
-        if (value < 1 || value > 64) return fail(MC_EINVAL, "hist_slices must be in 1..64");
-        h->hist_slices = (int)value;
-    } else if (!std::strcmp(key, "probe")) {
-        h->pmode = value != 0 ? 1 : 0;
-    } else if (!std::strcmp(key, "wave")) {
-        h->pwave = value != 0;
     } else if (!std::strcmp(key, "pnear")) {
         if (value < 0 || value > 128) return fail(MC_EINVAL, "pnear must be in 0..128");
         h->pnear = (int)value;
-    } else if (!std::strcmp(key, "debug")) {
-        h->debug = value != 0;
-    } else if (!std::strcmp(key, "prows")) {
-        if (value != 1 && value != 2 && value != 4) return fail(MC_EINVAL, "prows must be 1, 2 or 4");
-        h->prows = (int)value;
-    } else if (!std::strcmp(key, "graph")) {
-        h->use_graph = value != 0;
-    } else if (!std::strcmp(key, "overlap")) {
-        h->overlap = value != 0;
-    } else if (!std::strcmp(key, "bulk_rows")) {
-        if (value != 1 && value != 2) return fail(MC_EINVAL, "bulk_rows must be 1 or 2");
-        h->bulk_rows = (int)value;
-    } else if (!std::strcmp(key, "bulk_ctas")) {
-        if (value < 1 || value > 4) return fail(MC_EINVAL, "bulk_ctas must be in 1..4");
-        h->bulk_ctas = (int)value;
+    } else if (!std::strcmp(key, "wave")) {
+        h->pwave = value != 0;
+    } else if (!std::strcmp(key, "form")) {
+        // -1: the form the geometry allows; 0..2: that one or a more exact one (never a less exact one)
+        if (value < -1 || value > kFormCanon) return fail(MC_EINVAL, "form must be -1 (automatic), 0, 1 or 2");
+        if (value >= 0 && value < h->form_auto)
+            return fail(MC_EINVAL, "this geometry needs a more exact pair-distance form than the one requested");
+        h->form = value < 0 ? h->form_auto : (int)value;
     } else if (!std::strcmp(key, "uniform_path")) {
         h->allow_uniform = value != 0;
         h->uniform_d = h->allow_uniform && h->all_d_equal;
+    } else if (!std::strcmp(key, "stall_ms")) {
+        if (value < 0 || value > 3600000) return fail(MC_EINVAL, "stall_ms must be in 0..3600000 (0: no limit)");
+        h->p.wait_limit_ns = (unsigned long long)value * 1000000ull;
+    } else if (!std::strcmp(key, "hist_slices")) {
+        if (value < 1 || value > 64) return fail(MC_EINVAL, "hist_slices must be in 1..64");
+        h->hist_slices = (int)value;
+    } else if (!std::strcmp(key, "debug")) {
+        h->debug = value != 0;
+        if (!h->debug) h->pmode = 0;
+    } else if (!std::strcmp(key, "probe")) {
+        if (value < 0 || value > 2) return fail(MC_EINVAL, "probe must be 0, 1 or 2");
+        if (value != 0 && !h->debug) return fail(MC_EINVAL, "probe needs debug = 1 (its sweeps compute nothing meaningful)");
+        h->pmode = (int)value;
     } else {
         return fail(MC_EINVAL, std::string("unknown option ") + key);
     }
-    drop_graph(h);
+    return MC_OK;
+}
+
+int mc_get_option(mc_handle* h, const char* key, int64_t* value_host) {
+    if (!h || !key || !value_host) return fail(MC_EINVAL, "null argument");
+    if (!std::strcmp(key, "prows")) *value_host = h->prows;
+    else if (!std::strcmp(key, "far_cols")) *value_host = h->pfarcols;
+    else if (!std::strcmp(key, "pnear")) *value_host = h->pnear;
+    else if (!std::strcmp(key, "wave")) *value_host = h->pwave ? 1 : 0;
+    else if (!std::strcmp(key, "form")) *value_host = h->form;
+    else if (!std::strcmp(key, "form_auto")) *value_host = h->form_auto;
+    else if (!std::strcmp(key, "uniform_path")) *value_host = h->uniform_d ? 1 : 0;
+    else if (!std::strcmp(key, "stall_ms")) *value_host = (int64_t)(h->p.wait_limit_ns / 1000000ull);
+    else if (!std::strcmp(key, "hist_slices")) *value_host = h->hist_slices;
+    else if (!std::strcmp(key, "debug")) *value_host = h->debug ? 1 : 0;
+    else if (!std::strcmp(key, "probe")) *value_host = h->pmode;
+    else return fail(MC_EINVAL, std::string("unknown option ") + key);
     return MC_OK;
 }
 
@@ -773,14 +599,16 @@ int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers,
 }
 
 int mc_debug_peek(mc_handle* h, int32_t* out_host, int n) {
-    if (!h || !out_host || n > h->p.sy_n) return fail(MC_EINVAL, "bad argument");
+    // n > 0: the first n scheduling words; n < 0: the first -n 32-bit words of the diagnostic counters
+    if (!h || !out_host || n == 0 || n > h->p.sy_n || -(int64_t)n * 4 > (int64_t)(kDbgWords * 8))
+        return fail(MC_EINVAL, "bad argument");
     cudaStream_t s2;
     CUDA_TRY(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
-    if (n < 0) CUDA_TRY(cudaMemcpyAsync(out_host, h->ws + h->L.dbg, (size_t)(-n) * 4, cudaMemcpyDeviceToHost, s2));
-    else
-    CUDA_TRY(cudaMemcpyAsync(out_host, h->p.sy, (size_t)n * 4, cudaMemcpyDeviceToHost, s2));
-    CUDA_TRY(cudaStreamSynchronize(s2));
+    const void* src = n < 0 ? (const void*)(h->ws + h->L.dbg) : (const void*)h->p.sy;
+    const cudaError_t e = cudaMemcpyAsync(out_host, src, (size_t)(n < 0 ? -n : n) * 4, cudaMemcpyDeviceToHost, s2);
+    const cudaError_t e2 = cudaStreamSynchronize(s2);
     cudaStreamDestroy(s2);
+    if (e != cudaSuccess || e2 != cudaSuccess) return fail(MC_ECUDA, "mc_debug_peek: copy failed");
     return MC_OK;
 }
 

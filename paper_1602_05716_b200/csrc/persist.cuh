@@ -44,7 +44,8 @@ struct PArgs {
     int farcols;      // target columns per FAR item (multiple of 8)
     int nnear;        // worker CTAs 1..nnear serve FIX and DIAG only
     int nfar;         // number of FAR workers (0: do not round item counts to it)
-    int mode;         // 0 normal; 1 throughput probe: no chain, every CTA runs QU items over all columns but the chunk's own
+    int mode;         // 0 normal; 1 throughput probe: no chain, every CTA runs QU items over all columns but the chunk's own;
+                      // 2 watchdog test: the deciding warp never runs, so the sweep stalls
     int* sy;          // [kSyHdr + 3 * nchunks]: header, far_done, diag_done, fix_done
     long long* dbg;   // [16] diagnostic cycle counters (see mc_debug_counters), may be null
 };
@@ -90,22 +91,23 @@ __device__ __forceinline__ double2 ldcg2(const double2* p) {
     asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
     return v;
 }
-// Watchdog: no wait in this kernel may last longer than kWaitLimitNs.  A thread whose wait does
-// raises the abort flag (and DevState::stall, which the host reports as MC_ESTALL) and exits;
-// every other waiting thread sees the flag and exits too, so a scheduling bug can never hang the GPU.
-constexpr unsigned long long kWaitLimitNs = 2000000000ull;
+// Watchdog: no wait in this kernel may last longer than Params::wait_limit_ns (option "stall_ms",
+// default 2 s; 0 = no limit).  A thread whose wait does raises the abort flag (and DevState::stall,
+// which every synchronising call of the host reports as MC_ESTALL) and exits; every other waiting
+// thread sees the flag and exits too, so a scheduling bug can never hang the GPU.
 struct Watch {
     int* sy;
     DevState* st;
+    unsigned long long limit;
 };
 __device__ __forceinline__ unsigned long long global_ns() {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
-__device__ __noinline__ void wd_check(const Watch& w, unsigned long long t0) {
+static __device__ __noinline__ void wd_check(const Watch& w, unsigned long long t0) {
     if (*(volatile int*)(w.sy + kSyAbort) == 0) {
-        if (global_ns() - t0 < kWaitLimitNs) return;
+        if (w.limit == 0ull || global_ns() - t0 < w.limit) return;
         *(volatile int*)(w.sy + kSyAbort) = 1;
         *(volatile int*)(&w.st->stall) = 1;
         __threadfence();
@@ -180,7 +182,7 @@ __device__ __forceinline__ ChunkBufs chunk_bufs(const PArgs& a, int c) {
 namespace mcb {
 
 // exact overlap re-check with L2 loads (columns may have been rewritten by the chain during this kernel)
-__device__ __noinline__ int recheck_overlap_cg(const double2* xy, const double2* zq, const double* hh, double2 t,
+static __device__ __noinline__ int recheck_overlap_cg(const double2* xy, const double2* zq, const double* hh, double2 t,
                                                double tz, double hi, int v0, int v1, int cbeg, int gapv, int gap) {
     int ov = 0;
     for (int v = v0; v < v1; ++v) {
@@ -194,47 +196,118 @@ __device__ __noinline__ int recheck_overlap_cg(const double2* xy, const double2*
     return ov;
 }
 
-// Pair evaluation of the persistent kernel: 20 FP64-pipe instructions (22 if diameters differ) + 2 MUFU.
-//   r2o = |x_i|^2 + |x_j|^2 - 2 x_i.x_j           1 DADD + 3 DFMA   (n_j = |x_j|^2 is staged with the column)
-//   w   = 2 D.x_i + |D|^2 - 2 D.x_j               3 DFMA            (D = x~_i - x_i)
-//   r2n = r2o + w                                 1 DADD
-// The Gram form of r2o carries an absolute error of a few ulp of |x|^2 (<= 3e-13 for |x| <= 34 sigma):
-// far below the 2^-16 band inside which the veto is re-examined exactly, and 1e-13 relative in 1/r at contact.
-struct RowG {
-    double mx, my, mz;  // -2 x_i
-    double n;           // |x_i|^2
-    double ex, ey, ez;  // -2 D
-    double cp;          // 2 D.x_i + |D|^2
+// Pair evaluation (Eq. 2; Alg. 2) in three forms, chosen by mc_init from the
+// geometry so that the per-trial dE stays within 1e-10 of its natural scale:
+//  GRAM  (20 FP64-pipe instructions + 2 MUFU; 22 if diameters differ)    cavity_R / d_min <= 64
+//     r2o = |x_i|^2 + |x_j|^2 - 2 x_i.x_j       1 DADD + 3 DFMA   (|x_j|^2 is staged with the column)
+//     w   = 2 D.x_i + |D|^2 - 2 D.x_j           3 DFMA            (D = x~_i - x_i)
+//     r2n = r2o + w                             1 DADD
+//     absolute error of r2o: a few ulp(R^2), i.e. <= 5e-15 (R/r)^2 relative in 1/r
+//  DIFFW (22; 24)                                                         max_disp / d_min <= 64
+//     dx = x_i - x_j ... (3 DADD), r2o = fma(dz,dz,fma(dy,dy,dx dx)) (3), w = 2 D.dx + |D|^2 (3), r2n = r2o + w (1)
+//     r2o as the oracle forms it; r2n carries an absolute error of a few ulp((r_o + max_disp)^2)
+//  CANON (25; 27: the canonical count of SURVEY.md 8(d))                  any geometry
+//     both distances from rounded differences, exactly as reading G11 writes them
+// plus, in every form, 2 x 5 for the rsqrt refinements and 2 for the difference and the accumulate.
+// The overlap veto is an integer test off the FP64 pipe: a running signed minimum
+// (VIMNMX3, one per two pairs) of the high word of r2n (equal diameters) or of r2n - s_ij^2.
+// A negative r2n (possible in the GRAM form when the trial lands within ~1e-6 sigma of another centre) has a
+// negative high word and so wins the minimum: it reads as an overlap, never as a large distance.
+// A row whose minimum falls inside a narrow band around contact -- where the re-associated r2n could
+// differ from reading G11's evaluation order -- is re-examined exactly (recheck_overlap_cg).
+enum { kFormGram = 0, kFormDiffW = 1, kFormCanon = 2 };
+constexpr int kOvBand = 16;   // equal diameters: band of +-16 high-word steps (2^-16 relative) around s^2
+
+struct RowP {
+    double a0, a1, a2;  // GRAM: -2 x_i            DIFFW, CANON: x_i
+    double b0, b1, b2;  // GRAM: -2 D              DIFFW: 2 D            CANON: x~_i
+    double c0;          // GRAM: |x_i|^2           DIFFW: |D|^2
+    double c1;          // GRAM: 2 D.x_i + |D|^2
     double h;           // d/2
     double acc;
     int m;              // running minimum of the overlap key
 };
 
-template <bool UNIFORM>
-__device__ __forceinline__ int pair_eval_g(RowG& r, const double2 a, const double2 b, double nj, double hj) {
-    const double r2o = __fma_rn(r.mx, a.x, __fma_rn(r.my, a.y, __fma_rn(r.mz, b.x, __dadd_rn(r.n, nj))));
-    const double w = __fma_rn(r.ex, a.x, __fma_rn(r.ey, a.y, __fma_rn(r.ez, b.x, r.cp)));
-    const double r2n = __dadd_rn(r2o, w);
-    int key = __double2hiint(r2n);
-    if (!UNIFORM) {
+template <int FORM>
+__device__ __forceinline__ void row_init(RowP& r, double2 xyi, double zi, double2 txyi, double tzi, double ni, double hi) {
+    const double Dx = __dadd_rn(txyi.x, -xyi.x), Dy = __dadd_rn(txyi.y, -xyi.y), Dz = __dadd_rn(tzi, -zi);
+    if (FORM == kFormGram) {
+        r.a0 = __dmul_rn(-2.0, xyi.x); r.a1 = __dmul_rn(-2.0, xyi.y); r.a2 = __dmul_rn(-2.0, zi);
+        r.b0 = __dmul_rn(-2.0, Dx); r.b1 = __dmul_rn(-2.0, Dy); r.b2 = __dmul_rn(-2.0, Dz);
+        r.c0 = ni;
+        // 2 D.x_i + |D|^2 = D.(2 x_i + D)
+        r.c1 = __fma_rn(Dx, __fma_rn(2.0, xyi.x, Dx), __fma_rn(Dy, __fma_rn(2.0, xyi.y, Dy), __dmul_rn(Dz, __fma_rn(2.0, zi, Dz))));
+    } else if (FORM == kFormDiffW) {
+        r.a0 = xyi.x; r.a1 = xyi.y; r.a2 = zi;
+        r.b0 = __dadd_rn(Dx, Dx); r.b1 = __dadd_rn(Dy, Dy); r.b2 = __dadd_rn(Dz, Dz);
+        r.c0 = dist2(Dx, Dy, Dz);
+        r.c1 = 0.0;
+    } else {
+        r.a0 = xyi.x; r.a1 = xyi.y; r.a2 = zi;
+        r.b0 = txyi.x; r.b1 = txyi.y; r.b2 = tzi;
+        r.c0 = 0.0; r.c1 = 0.0;
+    }
+    r.h = hi;
+    r.acc = 0.0;
+    r.m = 0x7fffffff;
+}
+
+template <int FORM, bool UNIFORM>
+__device__ __forceinline__ int pair_eval(RowP& r, const double2 a, const double2 b, double nj, double hj) {
+    double r2o, r2n;
+    if (FORM == kFormGram) {
+        r2o = __fma_rn(r.a0, a.x, __fma_rn(r.a1, a.y, __fma_rn(r.a2, b.x, __dadd_rn(r.c0, nj))));
+        const double w = __fma_rn(r.b0, a.x, __fma_rn(r.b1, a.y, __fma_rn(r.b2, b.x, r.c1)));
+        r2n = __dadd_rn(r2o, w);
+    } else {
+        const double dx = __dadd_rn(r.a0, -a.x), dy = __dadd_rn(r.a1, -a.y), dz = __dadd_rn(r.a2, -b.x);
+        r2o = dist2(dx, dy, dz);
+        if (FORM == kFormDiffW) {
+            const double w = __fma_rn(r.b0, dx, __fma_rn(r.b1, dy, __fma_rn(r.b2, dz, r.c0)));
+            r2n = __dadd_rn(r2o, w);
+        } else {
+            r2n = dist2(__dadd_rn(r.b0, -a.x), __dadd_rn(r.b1, -a.y), __dadd_rn(r.b2, -b.x));
+        }
+    }
+    int key;
+    if (UNIFORM) {
+        key = __double2hiint(r2n);
+    } else {
         const double sij = __dadd_rn(r.h, hj);
-        key -= __double2hiint(__dmul_rn(sij, sij));
+        key = __double2hiint(__fma_rn(-sij, sij, r2n));   // sign and magnitude of r2n - s_ij^2
     }
     const double du = __dadd_rn(rsqrt_fast(r2n), -rsqrt_fast(r2o));
     r.acc = __fma_rn(b.y, du, r.acc);
     return key;
 }
 
+// What the running minimum m of a row's keys says about the veto: 1 overlap, 0 none, -1 inside the band
+// (re-examine exactly).  Signed order of the high words: any negative value (r2n < 0, or r2n - s^2 < 0)
+// is below every positive one, and among negative doubles the one closest to zero has the smallest word.
+template <bool UNIFORM>
+__device__ __forceinline__ int veto_from_min(int m, double h, double ov_tol) {
+    if (UNIFORM) {
+        if (m < 0) return 1;                                    // r2n itself came out negative: on top of a centre
+        const double s = __dadd_rn(h, h);
+        const int key = m - __double2hiint(__dmul_rn(s, s));     // both words in [0, 0x7ff00000): no wrap
+        return key < -kOvBand ? 1 : key > kOvBand ? 0 : -1;
+    }
+    const int tolhi = __double2hiint(ov_tol);
+    if (m >= tolhi) return 0;                                   // smallest r2n - s^2 is clearly positive
+    if (m < 0 && (m & 0x7fffffff) >= tolhi) return 1;           // the negative one closest to zero is clearly negative
+    return -1;
+}
+
 // FAR / FIX item: all rows of the chunk (ROWS per consumer thread) x virtual columns [v0, v1) of
 // the column space that starts at cbeg and skips [gap0, gap1).  Same inner loop as k_bulk; the
 // mbarrier ring persists across items (kring = stages used so far, identical in every thread).
-template <int ROWS, bool UNIFORM>
+template <int ROWS, bool UNIFORM, int FORM>
 __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned& kring, int row0, int nrows,
                                           int cbeg, int gap0, int gap1, int v0, int v1) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int gap = gap1 - gap0;
     const int gapv = gap0 - cbeg;
-    const Watch wd{p.sy, p.st};
+    const Watch wd{p.sy, p.st, p.wait_limit_ns};
 
     // producer state (thread 0 only): next stage to issue
     unsigned kp = kring;
@@ -245,10 +318,10 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
         const int a = cbeg + ((vp < gapv) ? vp : vp + gap);
         const unsigned s = kp % kStages;
         if (kp >= (unsigned)kStages) mbar_wait_wd(wd, &sh.empty_bar[s], ((kp / kStages) - 1) & 1);
-        mbar_arrive_expect_tx(&sh.full_bar[s], (uint32_t)cnt * (UNIFORM ? 40u : 48u));
+        mbar_arrive_expect_tx(&sh.full_bar[s], (uint32_t)cnt * (32u + (FORM == kFormGram ? 8u : 0u) + (UNIFORM ? 0u : 8u)));
         bulk_g2s(sh.u.w.stage[s].xy, p.xy + a, (uint32_t)cnt * 16u, &sh.full_bar[s]);
         bulk_g2s(sh.u.w.stage[s].zq, p.zq + a, (uint32_t)cnt * 16u, &sh.full_bar[s]);
-        bulk_g2s(sh.u.w.stage[s].n, p.nn + a, (uint32_t)cnt * 8u, &sh.full_bar[s]);
+        if (FORM == kFormGram) bulk_g2s(sh.u.w.stage[s].n, p.nn + a, (uint32_t)cnt * 8u, &sh.full_bar[s]);
         if (!UNIFORM) bulk_g2s(sh.u.w.stage[s].h, p.hh + a, (uint32_t)cnt * 8u, &sh.full_bar[s]);
         vp += cnt;
         ++kp;
@@ -258,23 +331,13 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
         for (int q = 0; q < kStages - 1 && vp < v1; ++q) issue();
     }
 
-    RowG R[ROWS];
+    RowP R[ROWS];
 #pragma unroll
     for (int u = 0; u < ROWS; ++u) {
         const int r = u * kBulkThreads + tid;
         const int i = row0 + (r < nrows ? r : 0);
         const double2 xyi = ldcg2(p.xy + i);
-        const double zi = __ldcg(&p.zq[i].x);
-        const double2 txyi = p.txy[i];
-        const double Dx = __dadd_rn(txyi.x, -xyi.x), Dy = __dadd_rn(txyi.y, -xyi.y), Dz = __dadd_rn(p.tz[i], -zi);
-        R[u].mx = __dmul_rn(-2.0, xyi.x); R[u].my = __dmul_rn(-2.0, xyi.y); R[u].mz = __dmul_rn(-2.0, zi);
-        R[u].n = __ldcg(p.nn + i);
-        R[u].ex = __dmul_rn(-2.0, Dx); R[u].ey = __dmul_rn(-2.0, Dy); R[u].ez = __dmul_rn(-2.0, Dz);
-        // 2 D.x_i + |D|^2 = D.(2 x_i + D)
-        R[u].cp = __fma_rn(Dx, __fma_rn(2.0, xyi.x, Dx), __fma_rn(Dy, __fma_rn(2.0, xyi.y, Dy), __dmul_rn(Dz, __fma_rn(2.0, zi, Dz))));
-        R[u].h = p.hh[i];
-        R[u].acc = 0.0;
-        R[u].m = 0x7fffffff;
+        row_init<FORM>(R[u], xyi, __ldcg(&p.zq[i].x), p.txy[i], p.tz[i], FORM == kFormGram ? __ldcg(p.nn + i) : 0.0, p.hh[i]);
     }
     const bool warp_live = warp * 32 < nrows;
 
@@ -294,11 +357,11 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
                     const double2 a0 = st.xy[j0 + jj], a1 = st.xy[j0 + jj + 1];
                     const double2 b0 = st.zq[j0 + jj], b1 = st.zq[j0 + jj + 1];
                     const double h0 = UNIFORM ? 0.0 : st.h[j0 + jj], h1 = UNIFORM ? 0.0 : st.h[j0 + jj + 1];
-                    const double n0 = st.n[j0 + jj], n1 = st.n[j0 + jj + 1];
+                    const double n0 = FORM == kFormGram ? st.n[j0 + jj] : 0.0, n1 = FORM == kFormGram ? st.n[j0 + jj + 1] : 0.0;
 #pragma unroll
                     for (int u = 0; u < ROWS; ++u) {
-                        const int k0 = pair_eval_g<UNIFORM>(R[u], a0, b0, n0, h0);
-                        const int k1 = pair_eval_g<UNIFORM>(R[u], a1, b1, n1, h1);
+                        const int k0 = pair_eval<FORM, UNIFORM>(R[u], a0, b0, n0, h0);
+                        const int k1 = pair_eval<FORM, UNIFORM>(R[u], a1, b1, n1, h1);
                         R[u].m = __vimin3_s32(R[u].m, k0, k1);
                     }
                 }
@@ -319,14 +382,9 @@ __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned
 #pragma unroll
     for (int u = 0; u < ROWS; ++u) {
         const int r = u * kBulkThreads + tid;
-        int key = R[u].m;
-        if (UNIFORM) {
-            const double s = __dadd_rn(R[u].h, R[u].h);
-            key -= __double2hiint(__dmul_rn(s, s));
-        }
-        int ov = key < 0 ? 1 : 0;
-        if (r < nrows && key >= -kOvBand && key <= kOvBand)
-            ov = recheck_overlap_cg(p.xy, p.zq, p.hh, p.txy[row0 + r], p.tz[row0 + r], R[u].h, v0, v1, cbeg, gapv, gap);
+        int ov = veto_from_min<UNIFORM>(R[u].m, R[u].h, p.ov_tol);
+        if (ov < 0)
+            ov = r < nrows ? recheck_overlap_cg(p.xy, p.zq, p.hh, p.txy[row0 + r], p.tz[row0 + r], R[u].h, v0, v1, cbeg, gapv, gap) : 0;
         if (r < nrows) accum_row(p, row0 + r, R[u].acc, ov);
     }
 }
@@ -346,7 +404,7 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
     const int slot = gt % kRing;
     HandOff& ho = sh.u.ho[slot];
     const unsigned apar = (unsigned)(c >> 1) & 1u;
-    const Watch wd{a.sy, a.p.st};
+    const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
 
     // base sum of all FAR, FIX and DIAG items of this row
     double E = accum_value(__ldcg(a.p.S1 + i), __ldcg(a.p.S2 + i));
@@ -406,7 +464,7 @@ __device__ __forceinline__ void chain_publisher(const PArgs& a, PShared& sh) {
     const int lane = threadIdx.x & 31;
     const Params& p = a.p;
     const int C = a.C, GPC = C / kGroup, ntfull = C / kTile;
-    const Watch wd{a.sy, a.p.st};
+    const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
     unsigned long long n_acc = 0, n_ov = 0, n_wall = 0, n_tie = 0;
     double e_lane = 0.0;
     for (int c = 0; c < a.nchunks; ++c) {
@@ -474,12 +532,12 @@ namespace mcb {
 // the chain CTA (a3/a4): Alg. 4; accept iff no veto and
 // l_B q_i sum + ln u < 0 (Eq. 1 in log form, strict; readings G3, G4)
 // ------------------------------------------------------------------------------------------
-__device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
+static __device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const Params& p = a.p;
     const int C = a.C;
     const int ntfull = C / kTile;
-    const Watch wd{a.sy, a.p.st};
+    const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
 
     if (warp == kHelpers + 1) {
         chain_publisher(a, sh);
@@ -511,6 +569,7 @@ __device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
     }
 
     // ---------------- the chain warp ----------------
+    if (a.mode == 2) return;   // watchdog test ("probe" = 2): nobody decides, the publisher's first wait runs into the limit
     long long w_first = 0, w_other = 0;
     const long long t_start = clock64();
     for (int c = 0; c < a.nchunks; ++c) {
@@ -657,11 +716,11 @@ __device__ __forceinline__ int ld_relaxed(const int* p) {
     return v;
 }
 
-__device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near, int* item) {
+static __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near, int* item) {
     const int C = a.C, GPC = C / kGroup, nfix = C / kFixCols, nmid = C / kMidCols;
     const int total_urgent = a.nchunks >= 2 ? nfix + (a.nchunks - 2) * (nfix + nmid) : 0;
     int* sy = a.sy;
-    const Watch wd{a.sy, a.p.st};
+    const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
     for (unsigned it = 1;; ++it) {
         if ((it & 1023u) == 0u) wd_check(wd, global_ns());   // no time limit of its own: leaves when another wait gave up
         // one round trip: five independent loads
@@ -699,23 +758,24 @@ __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near,
 }
 
 // DIAG item k of chunk c: 8 units (row tile, column tile), one per warp
-__device__ __noinline__ void diag_item(const PArgs& a, PShared& sh, int c, int k, int row0, int nrows) {
+static __device__ __noinline__ void diag_item(const PArgs& a, PShared& sh, int c, int k, int row0, int nrows) {
     const int warp = threadIdx.x >> 5;
     const ChunkBufs B = chunk_bufs(a, c);
     Params pc = a.p;
     pc.chunk = a.C;
     pc.Dblk = B.Dblk; pc.OVold = B.OVold; pc.OVnew = B.OVnew;
-    diag_unit<true>(pc, row0, nrows, k * 8 + warp, sh.u.w.cxy[warp], sh.u.w.czq[warp], sh.u.w.ctxy[warp],
+    diag_unit(pc, row0, nrows, k * 8 + warp, sh.u.w.cxy[warp], sh.u.w.czq[warp], sh.u.w.ctxy[warp],
                     sh.u.w.ch[warp], sh.u.w.ctz[warp]);
 }
 
-template <int ROWS, bool UNIFORM>
+template <int ROWS, bool UNIFORM, int FORM>
 __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     PShared& sh = *reinterpret_cast<PShared*>(smem_raw);
     const int tid = threadIdx.x, warp = tid >> 5;
     const Params& p = a.p;
     const int C = a.C;
+    if (*(volatile int*)&p.st->stall) return;   // a stalled sweep invalidated the state: no-op (k_trial did nothing either)
 
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) {
@@ -733,7 +793,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
             st_release(a.sy + kSyChainSm, (int)smid + 1);
         } else {
             int v;
-            const Watch wd{a.sy, a.p.st};
+            const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
             const unsigned long long t0 = global_ns();
             for (unsigned it = 1; (v = ld_acquire(a.sy + kSyChainSm)) == 0; ++it) {
                 __nanosleep(100);
@@ -791,7 +851,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
                 cb = row0 - (type == kItemMid ? 2 : 1) * C + k * w;
                 g0 = g1 = cb; v0 = 0; v1 = w;
             }
-            bulk_item<ROWS, UNIFORM>(p, sh, kring, row0, nrows, cb, g0, g1, v0, v1);
+            bulk_item<ROWS, UNIFORM, FORM>(p, sh, kring, row0, nrows, cb, g0, g1, v0, v1);
         }
         __syncthreads();
         if (tid == 0) {

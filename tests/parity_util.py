@@ -13,6 +13,21 @@ DE_RTOL = 1e-10      # north_star: per-trial dE within 1e-10 relative (scale of 
 POS_ATOL = 1e-12     # north_star: positions within 1e-12 sigma (they are in fact bit-identical)
 
 
+def record_margin(name, **values):
+    """Appends one line to gpurun_out/parity_margins.jsonl (the figures DESIGN.md section 3 quotes) and prints it."""
+    import json
+    import os
+    line = json.dumps({"case": name, **values})
+    print("parity margin:", line)
+    try:
+        d = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+        os.makedirs(d, exist_ok=True)
+        with open(os.path.join(d, "parity_margins.jsonl"), "a") as f:
+            f.write(line + "\n")
+    except OSError:
+        pass
+
+
 def make_pair(w, threads=1, validate=True, seed=None):
     """(gpu chain, oracle chain) for workload ``w`` from the same generated inputs."""
     from oracle import Oracle
@@ -44,8 +59,9 @@ def compare_last_sweep(g, o, tag="", first=0, count=None):
     return emax, int((diff & tie).sum())
 
 
-def lockstep(g, o, sweeps, tag="", every=1):
-    """Run both chains ``sweeps`` sweeps, comparing after every ``every`` sweeps.  Returns a summary."""
+def lockstep(g, o, sweeps, tag="", every=1, after_sweep=None):
+    """Run both chains ``sweeps`` sweeps, comparing after every ``every`` sweeps.  ``after_sweep(done)`` is
+    called once both chains are known to be in the same state.  Returns a summary."""
     worst, flips, done = 0.0, 0, 0
     while done < sweeps:
         n = min(every, sweeps - done)
@@ -62,6 +78,8 @@ def lockstep(g, o, sweeps, tag="", every=1):
         else:
             assert np.array_equal(pg, po), (f"{tag} sweep {done - 1}: positions differ "
                                             f"(max {np.abs(pg - po).max():.3e})")
+        if after_sweep is not None:
+            after_sweep(done)
     return {"max_dE_err": worst, "near_tie_flips": flips}
 
 

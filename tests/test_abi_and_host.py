@@ -52,12 +52,14 @@ def test_library_is_sm100a_native_with_bulk_async_copies(lib):
     out = subprocess.run(["cuobjdump", "-lelf", str(binding._LIBPATH)], capture_output=True, text=True).stdout
     assert "sm_100a" in out
     sass = subprocess.run(["cuobjdump", "-sass", str(binding._LIBPATH)], capture_output=True, text=True).stdout
-    bulk = [blk for blk in sass.split("Function :")[1:] if "k_bulk" in blk.splitlines()[0]]
-    assert bulk, "no k_bulk instantiation in the SASS"
-    for blk in bulk:
-        assert "UBLKCP" in blk          # cp.async.bulk (TMA unit) staging
+    sweep = [blk for blk in sass.split("Function :")[1:] if "k_sweep" in blk.splitlines()[0]]
+    assert len(sweep) == 18, "k_sweep: 3 row counts x 2 diameter paths x 3 pair-distance forms"
+    for blk in sweep:
+        assert "UBLKCP" in blk          # cp.async.bulk (TMA unit) staging of the column ring
+        assert "SYNCS" in blk           # mbarrier transactions
         assert "MUFU.RSQ64H" in blk     # FP64 rsqrt seed
         assert "DFMA" in blk
+        assert "VIMNMX3" in blk         # integer overlap veto off the FP64 pipe
 
 
 def test_host_argument_checks_need_no_gpu(lib):
@@ -133,6 +135,22 @@ def test_bench_helpers():
         pass
     s = c.summary()
     assert set(s) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+
+
+def test_gpus_flag_spawns_the_replicas_itself_outside_torchrun(monkeypatch):
+    """python bench.py --gpus N without WORLD_SIZE starts N ranks through torch.distributed.run on 127.0.0.1."""
+    sys.path.insert(0, ROOT)
+    import bench
+    seen = {}
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    monkeypatch.setattr(bench, "spawn_replicas", lambda n, argv: seen.update(n=n, argv=argv) or 0)
+    assert bench.main(["--gpus", "4", "--steps", "2", "--warmup", "3"]) == 0
+    assert seen == {"n": 4, "argv": ["--gpus", "4", "--steps", "2", "--warmup", "3"]}
+    cmd = []
+    monkeypatch.undo()
+    bench.spawn_replicas(2, ["--gpus", "2"], runner=lambda c: cmd.extend(c) or 0)
+    assert "torch.distributed.run" in cmd and "--nproc-per-node=2" in cmd and "127.0.0.1" in cmd
+    assert cmd[-2:] == ["--gpus", "2"] and cmd[-3].endswith("bench.py")
 
 
 def test_reference_arm_prints_one_json_line():
