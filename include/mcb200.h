@@ -75,7 +75,8 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
             const double* diameters_dev, double cavity_R, double bjerrum_length, double max_disp,
             uint64_t seed, void* workspace_dev, size_t workspace_bytes, void* stream, int validate);
 
-/* n full sequential sweeps (sweep indices s .. s+n-1), enqueued, no host sync.
+/* n full sequential sweeps (sweep indices s .. s+n-1), enqueued, no host sync: ONE cooperative launch of
+ * k_sweep per 1024 sweeps, trial generation included (PAPER.md:85-91 launched one kernel per cycle).
  * mc_sweep(a); mc_sweep(b) is bit-identical to mc_sweep(a+b).   PAPER.md:43-73, Alg. 1-5. */
 int mc_sweep(mc_handle* h, int64_t n);
 
@@ -131,15 +132,10 @@ const char* mc_last_error(void);
  * (thread-level DFMA/s).  Synchronises.  Not part of the hot path. */
 int mc_measure_fp64_peak(void* stream, double millis, double* dfma_per_second_host);
 
-/* Diagnostics for the roofline: runs ONE sweep (it advances the chain exactly as mc_sweep(h, 1)
- * does: same kernels, same arguments, bit-identical result) with CUDA events on the handle's stream
- * around each of its two launches.  Fills ms_host[MC_NKERNELS] with the device time per kernel,
- * launches_host[MC_NKERNELS] with the launch counts and pairs_host[MC_NKERNELS] with the pair
- * evaluations that count towards N(N-1) (no speculative or correction work).  Synchronises. */
-#define MC_K_TRIAL 0  /* k_trial: a1                                          */
-#define MC_K_SWEEP 1  /* k_sweep: a2-a4, the whole sweep in one cooperative launch */
-#define MC_NKERNELS 2
-int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_t* pairs_host);
+/* Diagnostics for the roofline: mc_sweep(h, n) (1 <= n <= 1024: one launch of k_sweep, which advances the chain
+ * exactly as mc_sweep does) with a CUDA event pair on the handle's stream around the launch; *ms_host = its
+ * device time.  The launch covers n N(N-1) pair evaluations that count.  Synchronises. */
+int mc_sweep_timed(mc_handle* h, int64_t n, double* ms_host);
 
 /* Diagnostics of the persistent sweep kernel (option "debug" = 1): SM-clock cycle counters of the
  * last sweep, out16_host[16]: [0] chain warp, whole sweep; [1] of which waiting for the first tile
@@ -155,8 +151,9 @@ int mc_debug_counters(mc_handle* h, int64_t* out16_host);
  * exactly once per chunk.  out4_host = {items, violations, widest item in columns, urgent items}. */
 int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers, int64_t* out4_host);
 
-/* Diagnostics: copies the first n ints of the sweep kernel's scheduling state (ticket counters,
- * progress counter, per-chunk completion counters; n <= 256 + 4 (N / 256 + 1)) -- or, for n < 0, the
+/* Diagnostics: copies the first n ints of the sweep kernel's scheduling state -- W = 256 + 4 (N / 256 + 1) live
+ * words (ticket counters, progress counter, per-chunk completion counters; zero between sweeps) followed by W
+ * words that hold their values at the end of the last completed sweep; n <= 2 W -- or, for n < 0, the
  * first -n 32-bit words of the diagnostic counters (-n <= 2080) -- to the host on a stream of its
  * own, without waiting for the handle's stream (usable while a sweep is running). */
 int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
@@ -170,8 +167,13 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
  *   "pnear"        0..128  worker CTAs that serve only urgent and in-chunk items (default 4)
  *   "wave"         0|1     round a chunk's FAR items to a multiple of the FAR workers (default 1)
  *   "form"         -1|0|1|2  pair-distance form (persist.cuh): -1 = by geometry (default): 0 GRAM if
- *                          cavity_R / d_min <= 64, else 1 DIFFW if max_disp / d_min <= 64, else 2 CANON;
- *                          a value below the automatic one is refused (it would break the dE bar)
+ *                          cavity_R / d_min <= 128, else 1 DIFFW if max_disp / d_min <= 64, else 2 CANON;
+ *                          a value below the automatic one is refused (it would break the dE bar) unless
+ *                          debug = 1 (measurements of that error)
+ *   "position_bits" 64|32  32: the paper's storage format (float4 positions): the current
+ *                          configuration is rounded to FP32 values (E_running := its from-scratch energy) and
+ *                          every later trial position is rounded to FP32 once more; all pair arithmetic stays
+ *                          FP64.  A different (equally valid) chain; the oracle has the same switch
  *   "uniform_path" 0|1     allow the equal-diameter specialisation (default 1)
  *   "stall_ms"     0..3600000  watchdog limit per wait of the sweep kernel in ms (default 2000; 0 = none;
  *                          raise it under a profiler, a sanitizer or GPU time-slicing)

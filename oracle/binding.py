@@ -58,6 +58,7 @@ def load_oracle():
     lib.oracle_set_threads.argtypes = [vp, C.c_int]
     lib.oracle_sweep.argtypes = [vp, C.c_int64]
     lib.oracle_partial_sweep.argtypes = [vp, C.c_int64, C.c_int64]
+    lib.oracle_set_position_bits.argtypes = [vp, C.c_int]
     lib.oracle_energy.argtypes = [vp, dp]
     lib.oracle_pair_hist.argtypes = [vp, C.c_double, C.c_int, C.c_double, u64p, u64p]
     lib.oracle_get_positions.argtypes = [vp, dp]
@@ -125,6 +126,10 @@ class Oracle:
 
     def set_threads(self, n):
         self._ck(self._lib.oracle_set_threads(self._h, int(n)))
+
+    def set_position_bits(self, bits):
+        """32: positions are held as FP32 values, arithmetic stays FP64; 64: the default."""
+        self._ck(self._lib.oracle_set_position_bits(self._h, int(bits)))
 
     def sweep(self, n=1):
         self._ck(self._lib.oracle_sweep(self._h, int(n)))

@@ -80,6 +80,9 @@ struct Handle {
     double R = 0, lB = 0, max_disp = 0;
     uint64_t seed = 0, sweep = 0;
     int threads = 1;
+    // 64: positions are FP64 (north star, reading G8).  32: the paper's storage format -- every position the
+    // chain holds is an FP32 value (float4 X_dev); all arithmetic on them stays FP64.
+    int pos_bits = 64;
     // statistics since init
     uint64_t n_accept = 0, n_veto_overlap = 0, n_veto_wall = 0, n_near_tie = 0;
     double E_run = 0;
@@ -113,6 +116,9 @@ Trial make_trial(const Handle& h, int64_t i) {
     t.tx = std::fma(ux - 0.5, D, h.x[i]);
     t.ty = std::fma(uy - 0.5, D, h.y[i]);
     t.tz = std::fma(uz - 0.5, D, h.z[i]);
+    if (h.pos_bits == 32) {   // the proposed position is stored as FP32: one more rounding, to nearest
+        t.tx = (double)(float)t.tx; t.ty = (double)(float)t.ty; t.tz = (double)(float)t.tz;
+    }
     const double a = h.R - 0.5 * h.d[i];
     const double rr = std::fma(t.tz, t.tz, std::fma(t.ty, t.ty, t.tx * t.tx));
     t.wall_veto = rr > a * a;
@@ -263,6 +269,22 @@ void oracle_free(void* hp) { delete (Handle*)hp; }
 int oracle_set_threads(void* hp, int n) {
     if (!hp || n < 1) return ORACLE_EINVAL;
     ((Handle*)hp)->threads = n;
+    return ORACLE_OK;
+}
+
+// Position storage precision: bits = 32 rounds the current positions to
+// FP32 (to nearest) and makes every later trial position an FP32 value; E_running is recomputed from scratch.
+// bits = 64 only switches the rounding of later trials off.
+int oracle_set_position_bits(void* hp, int bits) {
+    if (!hp || (bits != 32 && bits != 64)) return ORACLE_EINVAL;
+    Handle& h = *(Handle*)hp;
+    h.pos_bits = bits;
+    if (bits == 32) {
+        for (int64_t i = 0; i < h.N; ++i) {
+            h.x[i] = (double)(float)h.x[i]; h.y[i] = (double)(float)h.y[i]; h.z[i] = (double)(float)h.z[i];
+        }
+        h.E_run = total_energy(h);
+    }
     return ORACLE_OK;
 }
 

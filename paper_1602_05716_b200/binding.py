@@ -57,7 +57,7 @@ def load_library() -> C.CDLL:
     lib.mc_sweep.argtypes = [vp, i64]
     lib.mc_energy.argtypes = [vp, C.POINTER(dbl)]
     lib.mc_energy_dev.argtypes = [vp, vp]
-    lib.mc_sweep_timed.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64), C.POINTER(i64)]
+    lib.mc_sweep_timed.argtypes = [vp, i64, C.POINTER(dbl)]
     lib.mc_pair_hist.argtypes = [vp, dbl, C.c_int, dbl, vp, vp]
     lib.mc_sweep_host.argtypes = [vp, i64, vp, C.POINTER(dbl), vp, C.POINTER(mc_stats)]
     lib.mc_get_positions.argtypes = [vp, vp]
@@ -176,14 +176,11 @@ class MCSystem:
         _check(self._lib.mc_energy_dev(self._h, out.data_ptr()))
         return out
 
-    KERNEL_CLASSES = ("k_trial", "k_sweep")
-
-    def mc_sweep_timed(self) -> dict:
-        """One sweep with an event pair around every launch: {class: (ms, launches, pair evals)}."""
-        n = len(self.KERNEL_CLASSES)
-        ms, cnt, pairs = (C.c_double * n)(), (C.c_int64 * n)(), (C.c_int64 * n)()
-        _check(self._lib.mc_sweep_timed(self._h, ms, cnt, pairs))
-        return {k: (ms[i], cnt[i], pairs[i]) for i, k in enumerate(self.KERNEL_CLASSES)}
+    def mc_sweep_timed(self, n: int = 1) -> float:
+        """mc_sweep(n) as one launch of k_sweep with an event pair around it: its device time in ms."""
+        ms = C.c_double()
+        _check(self._lib.mc_sweep_timed(self._h, int(n), C.byref(ms)))
+        return ms.value
 
     def mc_pair_hist(self, bin_width, nbins, centre_rmax, hist=None, n_centres=None):
         if hist is None:

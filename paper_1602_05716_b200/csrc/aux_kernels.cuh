@@ -1,46 +1,8 @@
-// aux_kernels.cuh -- the kernels of libmcb200 around the sweep (sm_100a): trial generation (a1), packing and
-// accessors, from-scratch energy (a5), pair histograms (a6), the FP64 peak probe.  Included by mcb200.cu only.
+// aux_kernels.cuh -- the kernels of libmcb200 around the sweep (sm_100a): packing and accessors, from-scratch energy (a5), pair histograms (a6), the FP64 peak probe.  Included by mcb200.cu only.
 #pragma once
 #include "kernels.cuh"
 
 namespace mcb {
-
-// ------------------------------------------------------------------------------------------
-// a1: trial generation.  Alg. 1 + old position (G1), D = 2 max_disp (G2),
-// Philox keyed by (seed; particle, sweep, tag) (G9), hard wall (G6).
-// ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_trial(Params p) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p.st->stall) return;   // after a stalled sweep every later sweep is a no-op until the state is replaced
-    for (int j = i; j < p.sy_n; j += gridDim.x * blockDim.x) p.sy[j] = 0;
-    if (i >= p.Np) return;
-    p.S1[i] = 0ll; p.S2[i] = 0ll; p.ovc[i] = 0;
-    const double2 xy = p.xy[i];
-    const double2 zq = p.zq[i];
-    if (i >= p.N) {  // ghost padding: never moves
-        p.txy[i] = xy; p.tz[i] = zq.x; p.lnu[i] = 0.0; p.wall[i] = (unsigned char)kFlagWall;
-        return;
-    }
-    const unsigned long long s = p.st->sweep;
-    const uint32_t k0 = (uint32_t)p.seed, k1 = (uint32_t)(p.seed >> 32);
-    uint32_t A[4], B[4];
-    philox4x32_10((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, k0, k1, A);
-    philox4x32_10((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 1u, k0, k1, B);
-    const double ux = uniform_open01(A[0], A[1]);
-    const double uy = uniform_open01(A[2], A[3]);
-    const double uz = uniform_open01(B[0], B[1]);
-    const double ua = uniform_open01(B[2], B[3]);
-    const double D = __dmul_rn(2.0, p.max_disp);
-    const double tx = __fma_rn(__dadd_rn(ux, -0.5), D, xy.x);
-    const double ty = __fma_rn(__dadd_rn(uy, -0.5), D, xy.y);
-    const double tz = __fma_rn(__dadd_rn(uz, -0.5), D, zq.x);
-    const double a = __dadd_rn(p.R, -p.hh[i]);
-    const double rr = dist2(tx, ty, tz);
-    p.txy[i] = make_double2(tx, ty);
-    p.tz[i] = tz;
-    p.lnu[i] = log(ua);
-    p.wall[i] = (rr > __dmul_rn(a, a)) ? (unsigned char)kFlagWall : (unsigned char)0;
-}
 
 // ------------------------------------------------------------------------------------------
 // packing between the caller's SoA [3][N] and the workspace layout
@@ -65,6 +27,18 @@ __global__ void k_pack(Params p, const double* pos, const double* q, const doubl
         p.hh[i] = 0.0;
         p.lbq[i] = 0.0;
     }
+}
+
+// FP32-position variant: round the configuration to FP32 values, to nearest
+__global__ void k_round_positions(Params p) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.N) return;
+    const double2 xy = p.xy[i];
+    const double x = (double)__double2float_rn(xy.x), y = (double)__double2float_rn(xy.y);
+    const double z = (double)__double2float_rn(p.zq[i].x);
+    p.xy[i] = make_double2(x, y);
+    p.zq[i].x = z;
+    p.nn[i] = dist2(x, y, z);
 }
 
 __global__ void k_unpack(Params p, double* pos) {
@@ -114,17 +88,18 @@ __global__ void k_check_particles(Params p, const double* d) {
 
 // ------------------------------------------------------------------------------------------
 // a5: from-scratch energy (and the overlap check of mc_init): E = l_B sum_{i<j} q_i q_j / r_ij.
-// The upper triangle is cut into units of 1024 rows x 1024 columns (4 column tiles of 256); one CTA
-// per unit, 4 rows per thread, columns staged through shared memory, 10 FP64-pipe instructions per
-// pair.  Units on the diagonal test j > i per pair.  Every CTA reduces its rows in a fixed order and
-// writes one partial; k_energy_reduce adds the partials in index order.
+// The upper triangle is cut into units of 1024 rows x 256 columns (8320 at N = 65536: the last, partly
+// filled wave of CTAs is 1/28 of the run); one CTA per unit, 4 rows per thread, columns staged through
+// shared memory, 10 FP64-pipe instructions per pair.  Units inside the diagonal 1024 x 1024 blocks test
+// j > i per pair.  Every CTA reduces its rows in a fixed order and writes one partial; k_energy_reduce
+// adds the partials in index order.
 // ------------------------------------------------------------------------------------------
 constexpr int kERows = 4, kEBlock = 256 * kERows, kETile = 256;
 
 __host__ __device__ inline int energy_units(int Np) {
     const int nrb = (Np + kEBlock - 1) / kEBlock;
     int n = 0;
-    for (int rb = 0; rb < nrb; ++rb) n += ((Np - rb * kEBlock) + kEBlock - 1) / kEBlock;
+    for (int rb = 0; rb < nrb; ++rb) n += ((Np - rb * kEBlock) + kETile - 1) / kETile;
     return n;
 }
 
@@ -134,15 +109,15 @@ __global__ void __launch_bounds__(256, 2) k_energy(Params p, double* part) {
     __shared__ double sh[kETile], sn[kETile];
     __shared__ double red[8];
     const int tid = threadIdx.x;
-    // unit -> (row block rb, column block cb >= rb)
+    // unit -> (row block rb, column tile ct of the columns from the row block's first row on)
     int unit = blockIdx.x, rb = 0;
     for (;;) {
-        const int n = ((p.Np - rb * kEBlock) + kEBlock - 1) / kEBlock;
+        const int n = ((p.Np - rb * kEBlock) + kETile - 1) / kETile;
         if (unit < n) break;
         unit -= n;
         ++rb;
     }
-    const int cb = rb + unit;
+    const int ct = unit;
     // off the diagonal: r^2 = |x_i|^2 + |x_j|^2 - 2 x_i.x_j (1 DADD + 3 DFMA; |x|^2 is kept per particle, p.nn),
     // 10 FP64-pipe instructions per pair; on the diagonal and in the overlap check of mc_init the
     // differences are formed explicitly (reading G11's evaluation order)
@@ -159,15 +134,13 @@ __global__ void __launch_bounds__(256, 2) k_energy(Params p, double* part) {
         nn[u] = live ? p.nn[i] : 9.0e18;
         acc[u] = 0.0;
     }
-    const bool diagonal = cb == rb;
+    const bool diagonal = ct < kEBlock / kETile;
     double mx[kERows], my[kERows], mz[kERows];
 #pragma unroll
     for (int u = 0; u < kERows; ++u) { mx[u] = __dmul_rn(-2.0, x[u]); my[u] = __dmul_rn(-2.0, y[u]); mz[u] = __dmul_rn(-2.0, z[u]); }
-    for (int ct = 0; ct < kEBlock / kETile; ++ct) {
-        const int j0 = cb * kEBlock + ct * kETile;
-        if (j0 >= p.Np) break;
+    {
+        const int j0 = rb * kEBlock + ct * kETile;
         const int cnt = min(kETile, p.Np - j0);
-        __syncthreads();
         if (tid < cnt) {
             sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; sn[tid] = p.nn[j0 + tid];
             if (CHECK) sh[tid] = p.hh[j0 + tid];

@@ -24,7 +24,8 @@ struct DevState {
     double E_run;
     int err;        // validation result (0 ok, MC_E* otherwise)
     int d_differs;  // set by k_check_particles if not all diameters are equal
-    int stall;      // set by the persistent sweep kernel's watchdog (a wait exceeded its time limit)
+    int stall;      // set by the sweep kernel's watchdog (a wait exceeded its time limit)
+    int sched_mismatch;   // sweeps whose per-chunk completion counters did not equal the plan's item counts (must stay 0)
     unsigned long long dmin_bits;   // bit pattern of the smallest diameter (k_check_particles; ~0 before)
 };
 

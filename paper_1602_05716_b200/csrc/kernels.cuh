@@ -22,11 +22,12 @@ struct Params {
     DevState* st;
     double R, lB, max_disp;
     unsigned long long seed;
-    int* sy; int sy_n;         // scheduling state of the persistent sweep kernel (zeroed by k_trial)
+    int* sy; int sy_n;         // scheduling state of the sweep kernel (zero between sweeps)
     long long* S1; long long* S2; int* ovc;   // [Np] per-row fixed-point sums / overlap counts (persistent kernel)
     double* nn;                // [Np] |x_i|^2 of the current positions (Gram form of the pair distance)
     double ov_tol;             // half-width of the band around contact inside which a veto is re-examined exactly
     unsigned long long wait_limit_ns;   // watchdog limit per wait of the sweep kernel (0: none)
+    int pos_bits;              // 64, or 32: every position the chain holds is an FP32 value, arithmetic stays FP64
 };
 
 // Order-independent accumulation of a row's partial sums (persistent kernel): the double is split
@@ -43,6 +44,42 @@ __device__ __forceinline__ void accum_row(const Params& p, int i, double acc, in
 }
 __device__ __forceinline__ double accum_value(long long s1, long long s2) {
     return __fma_rn(__ll2double_rn(s2), 0x1.0p-70, __dmul_rn(__ll2double_rn(s1), 0x1.0p-20));
+}
+
+// ------------------------------------------------------------------------------------------
+// a1: trial generation for particle i of sweep s.  Alg. 1 + old position (G1), D = 2 max_disp
+// (G2), Philox keyed by (seed; particle, sweep, tag) (G9), hard wall (G6).  Also clears the row's
+// accumulators.  Runs inside the sweep kernel (persist.cuh: trial_phase), all threads of the grid.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void trial_one(const Params& p, int i, unsigned long long s) {
+    p.S1[i] = 0ll; p.S2[i] = 0ll; p.ovc[i] = 0;
+    const double2 xy = p.xy[i];
+    const double2 zq = p.zq[i];
+    if (i >= p.N) {  // ghost padding: never moves
+        p.txy[i] = xy; p.tz[i] = zq.x; p.lnu[i] = 0.0; p.wall[i] = (unsigned char)kFlagWall;
+        return;
+    }
+    const uint32_t k0 = (uint32_t)p.seed, k1 = (uint32_t)(p.seed >> 32);
+    uint32_t A[4], B[4];
+    philox4x32_10((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, k0, k1, A);
+    philox4x32_10((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 1u, k0, k1, B);
+    const double ux = uniform_open01(A[0], A[1]);
+    const double uy = uniform_open01(A[2], A[3]);
+    const double uz = uniform_open01(B[0], B[1]);
+    const double ua = uniform_open01(B[2], B[3]);
+    const double D = __dmul_rn(2.0, p.max_disp);
+    double tx = __fma_rn(__dadd_rn(ux, -0.5), D, xy.x);
+    double ty = __fma_rn(__dadd_rn(uy, -0.5), D, xy.y);
+    double tz = __fma_rn(__dadd_rn(uz, -0.5), D, zq.x);
+    if (p.pos_bits == 32) {   // the proposed position is stored as FP32: one more rounding, to nearest
+        tx = (double)__double2float_rn(tx); ty = (double)__double2float_rn(ty); tz = (double)__double2float_rn(tz);
+    }
+    const double a = __dadd_rn(p.R, -p.hh[i]);
+    const double rr = dist2(tx, ty, tz);
+    p.txy[i] = make_double2(tx, ty);
+    p.tz[i] = tz;
+    p.lnu[i] = log(ua);
+    p.wall[i] = (rr > __dmul_rn(a, a)) ? (unsigned char)kFlagWall : (unsigned char)0;
 }
 
 // ------------------------------------------------------------------------------------------

@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -37,7 +38,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t xy, zq, hh, lbq, txy, tz, lnu, wall, Dblk, OVold, OVnew, log_dE, log_flags,
-        st, epart, centres, ccount, stage_pos, S1, S2, ovc, nn, sy, dbg, hcode, hcount, hcursor, hsxy, hszq, hbbox, total;
+        st, epart, centres, ccount, stage_pos, S1, S2, ovc, nn, sy, gbar, dbg, hcode, hcount, hcursor, hsxy, hszq, hbbox, total;
 };
 
 int padded(int64_t N) { return (int)((N + kTile - 1) / kTile * kTile); }
@@ -54,7 +55,8 @@ Layout make_layout(int64_t N) {
     L.Dblk = take(2 * (nt * (nt + 1) / 2) * kTile * kTile * 8);
     L.OVold = take((size_t)2 * kChunkMax * nt * 4); L.OVnew = take((size_t)2 * kChunkMax * nt * 4);
     L.S1 = take(Np * 8); L.S2 = take(Np * 8); L.ovc = take(Np * 4); L.nn = take(Np * 8);
-    L.sy = take((size_t)(kSyHdr + 4 * (Np / 256 + 1)) * 4);
+    L.sy = take((size_t)2 * (kSyHdr + 4 * (Np / 256 + 1)) * 4);   // live words + snapshot of the last completed sweep
+    L.gbar = take(256);
     L.dbg = take(kDbgWords * 8);
     L.hcode = take(Np * 4); L.hcount = take((size_t)kCells * 4); L.hcursor = take((size_t)kCells * 4);
     L.hsxy = take(Np * 16); L.hszq = take(Np * 16); L.hbbox = take((Np / 256 + 1) * 4 * 6 * 8);
@@ -100,10 +102,12 @@ struct mc_handle {
 namespace {
 
 // geometry limits of the pair-distance forms (persist.cuh)
-constexpr double kGramMaxRatio = 64.0;    // GRAM  needs cavity_R / d_min <= 64
+constexpr double kGramMaxRatio = 128.0;   // GRAM  needs cavity_R / d_min <= 128 (measured: 2e-12 there, 6e-11 at 500)
 constexpr double kDiffWMaxRatio = 64.0;   // DIFFW needs max_disp / d_min <= 64
 
-int launch_sweep(mc_handle* h, cudaStream_t s) {
+// One cooperative launch that runs nsweeps full sweeps (a1-a4 each): trial generation, the pair sums, the
+// sequential resolution and the commit all happen inside k_sweep (persist.cuh).
+int launch_sweep(mc_handle* h, cudaStream_t s, int nsweeps) {
     SweepLaunch L{};
     L.rows = h->prows;
     L.uniform = h->uniform_d;
@@ -128,7 +132,9 @@ int launch_sweep(mc_handle* h, cudaStream_t s) {
     a.farcols = h->pfarcols;
     a.mode = h->pmode;
     a.nfar = h->pwave ? std::max(1, h->pgrid - 2 - a.nnear) : 0;
+    a.nsweeps = nsweeps;
     a.sy = h->p.sy;
+    a.gbar = (int*)(h->ws + h->L.gbar);
     a.dbg = h->debug ? (long long*)(h->ws + h->L.dbg) : nullptr;
     if (a.dbg) CUDA_TRY(cudaMemsetAsync(a.dbg, 0, kDbgWords * 8, s));
     L.grid = h->pgrid;
@@ -137,12 +143,13 @@ int launch_sweep(mc_handle* h, cudaStream_t s) {
     return MC_OK;
 }
 
-// one sweep: k_trial (a1; also resets the scheduling words and the row accumulators), then k_sweep (a2-a4)
-int enqueue_sweep(mc_handle* h, cudaStream_t s) {
-    const Params& p = h->p;
-    k_trial<<<(p.Np + 255) / 256, 256, 0, s>>>(p);
-    CUDA_TRY(cudaGetLastError());
-    return launch_sweep(h, s);
+constexpr int64_t kMaxSweepsPerLaunch = 1024;   // keeps a single launch bounded in time
+
+// after a stalled sweep (or before the first one) the scheduling words and the grid barrier must be clean
+int reset_scheduling(mc_handle* h) {
+    CUDA_TRY(cudaMemsetAsync(h->p.sy, 0, (size_t)h->p.sy_n * 4, h->stream));
+    CUDA_TRY(cudaMemsetAsync(h->ws + h->L.gbar, 0, 256, h->stream));
+    return MC_OK;
 }
 
 int enqueue_energy(mc_handle* h, double* out_dev, int set_running, int check_overlap) {
@@ -161,10 +168,14 @@ int enqueue_energy(mc_handle* h, double* out_dev, int set_running, int check_ove
 // Waits for the handle's stream and reports a stalled sweep (the watchdog of persist.cuh): after
 // MC_ESTALL the configuration is invalid until mc_set_positions / mc_set_state replaces it.
 int sync_and_check(mc_handle* h) {
-    int stall = 0;
-    CUDA_TRY(cudaMemcpyAsync(&stall, &h->p.st->stall, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    int flags[2] = {0, 0};   // DevState::stall, DevState::sched_mismatch (adjacent)
+    static_assert(offsetof(DevState, sched_mismatch) == offsetof(DevState, stall) + sizeof(int), "layout");
+    CUDA_TRY(cudaMemcpyAsync(flags, &h->p.st->stall, sizeof(flags), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
-    if (stall)
+    if (flags[1])
+        return fail(MC_ESTALL, "internal error: a sweep's completion counters did not match its plan (" +
+                               std::to_string(flags[1]) + " sweeps); the state is not to be trusted");
+    if (flags[0])
         return fail(MC_ESTALL, "a sweep stalled (a wait of the sweep kernel exceeded stall_ms); the state is invalid "
                                "until mc_set_positions or mc_set_state replaces it");
     return MC_OK;
@@ -224,6 +235,7 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     h->prows = p.Np >= 16384 ? 4 : (p.Np >= 2048 ? 2 : 1);
     p.R = cavity_R; p.lB = bjerrum_length; p.max_disp = max_disp; p.seed = seed;
     p.wait_limit_ns = 2000000000ull;
+    p.pos_bits = 64;
     h->epart = (double*)(w + L.epart);
     h->centres = (int*)(w + L.centres);
     h->ccount = (int*)(w + L.ccount);
@@ -277,11 +289,13 @@ int mc_free(mc_handle* h) {
 
 int mc_sweep(mc_handle* h, int64_t n) {
     if (!h || n < 0) return fail(MC_EINVAL, "bad handle or n < 0");
-    for (int64_t s = 0; s < n; ++s) {
-        const int rc = enqueue_sweep(h, h->stream);
+    while (n > 0) {
+        const int64_t m = std::min(n, kMaxSweepsPerLaunch);
+        const int rc = launch_sweep(h, h->stream, (int)m);
         if (rc != MC_OK) return rc;
+        h->launches += 1;
+        n -= m;
     }
-    h->launches += 2 * (uint64_t)n;
     return MC_OK;
 }
 
@@ -299,28 +313,20 @@ int mc_energy_dev(mc_handle* h, double* E_dev) {
     return enqueue_energy(h, E_dev, 0, 0);
 }
 
-int mc_sweep_timed(mc_handle* h, double* ms_host, int64_t* launches_host, int64_t* pairs_host) {
-    if (!h || !ms_host || !launches_host || !pairs_host) return fail(MC_EINVAL, "null argument");
-    for (int k = 0; k < MC_NKERNELS; ++k) { ms_host[k] = 0.0; launches_host[k] = 0; pairs_host[k] = 0; }
-    cudaEvent_t ev[3];
+int mc_sweep_timed(mc_handle* h, int64_t n, double* ms_host) {
+    if (!h || !ms_host || n < 1 || n > kMaxSweepsPerLaunch) return fail(MC_EINVAL, "null argument or n outside 1..1024");
+    cudaEvent_t ev[2];
     for (auto& x : ev) CUDA_TRY(cudaEventCreate(&x));
-    const Params& p = h->p;
-    // the launches of mc_sweep(h, 1), with an event between the two kernels
     CUDA_TRY(cudaEventRecord(ev[0], h->stream));
-    k_trial<<<(p.Np + 255) / 256, 256, 0, h->stream>>>(p);
-    CUDA_TRY(cudaEventRecord(ev[1], h->stream));
-    const int rc = launch_sweep(h, h->stream);
+    const int rc = launch_sweep(h, h->stream, (int)n);       // the launch of mc_sweep(h, n)
     if (rc != MC_OK) return rc;
-    CUDA_TRY(cudaEventRecord(ev[2], h->stream));
-    h->launches += 2;
+    CUDA_TRY(cudaEventRecord(ev[1], h->stream));
+    h->launches += 1;
     const int rs = sync_and_check(h);
-    float a = 0.f, b = 0.f;
-    CUDA_TRY(cudaEventElapsedTime(&a, ev[0], ev[1]));
-    CUDA_TRY(cudaEventElapsedTime(&b, ev[1], ev[2]));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, ev[0], ev[1]));
     for (auto& x : ev) cudaEventDestroy(x);
-    ms_host[MC_K_TRIAL] = a; launches_host[MC_K_TRIAL] = 1;
-    ms_host[MC_K_SWEEP] = b; launches_host[MC_K_SWEEP] = 1;
-    pairs_host[MC_K_SWEEP] = (int64_t)p.N * (int64_t)(p.N - 1);
+    *ms_host = ms;
     return rs;
 }
 
@@ -382,6 +388,8 @@ int mc_set_positions(mc_handle* h, const double* pos_dev) {
     k_set_state<<<1, 1, 0, h->stream>>>(h->p.st, 0ull, 0, 0.0, 0);
     h->launches += 2;
     CUDA_TRY(cudaGetLastError());
+    const int rc = reset_scheduling(h);
+    if (rc != MC_OK) return rc;
     return enqueue_energy(h, nullptr, 1, 0);
 }
 
@@ -392,7 +400,7 @@ int mc_set_state(mc_handle* h, const double* pos_dev, uint64_t sweep_index, doub
     k_set_state<<<1, 1, 0, h->stream>>>(h->p.st, (unsigned long long)sweep_index, 1, E_running, 1);
     h->launches += 2;
     CUDA_TRY(cudaGetLastError());
-    return MC_OK;
+    return reset_scheduling(h);
 }
 
 int mc_get_sweep_index(mc_handle* h, uint64_t* s_host) {
@@ -420,7 +428,7 @@ int mc_get_stats(mc_handle* h, mc_stats* stats_host) {
     stats_host->accepted = st.accepted; stats_host->veto_overlap = st.veto_overlap;
     stats_host->veto_wall = st.veto_wall; stats_host->near_ties = st.near_ties;
     stats_host->E_running = st.E_run;
-    if (st.stall) return sync_and_check(h);
+    if (st.stall || st.sched_mismatch) return sync_and_check(h);
     return MC_OK;
 }
 
@@ -444,7 +452,7 @@ int mc_sweep_host(mc_handle* h, int64_t n, const double* pos_in_host, const doub
             k_pack<<<(h->p.Np + 255) / 256, 256, 0, h->stream>>>(h->p, h->stage_pos, nullptr, nullptr);
             k_set_state<<<1, 1, 0, h->stream>>>(h->p.st, 0ull, 0, *E_running_in, 1);
             h->launches += 2;
-            rc = cudaGetLastError() == cudaSuccess ? MC_OK : fail(MC_ECUDA, "mc_sweep_host: launch failed");
+            rc = cudaGetLastError() == cudaSuccess ? reset_scheduling(h) : fail(MC_ECUDA, "mc_sweep_host: launch failed");
         } else {
             rc = mc_set_positions(h, h->stage_pos);
         }
@@ -508,9 +516,18 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     } else if (!std::strcmp(key, "form")) {
         // -1: the form the geometry allows; 0..2: that one or a more exact one (never a less exact one)
         if (value < -1 || value > kFormCanon) return fail(MC_EINVAL, "form must be -1 (automatic), 0, 1 or 2");
-        if (value >= 0 && value < h->form_auto)
+        if (value >= 0 && value < h->form_auto && !h->debug)
             return fail(MC_EINVAL, "this geometry needs a more exact pair-distance form than the one requested");
         h->form = value < 0 ? h->form_auto : (int)value;
+    } else if (!std::strcmp(key, "position_bits")) {
+        if (value != 32 && value != 64) return fail(MC_EINVAL, "position_bits must be 32 or 64");
+        h->p.pos_bits = (int)value;
+        if (value == 32) {   // round the current configuration; E_running := its from-scratch energy
+            k_round_positions<<<(h->p.N + 255) / 256, 256, 0, h->stream>>>(h->p);
+            h->launches += 1;
+            CUDA_TRY(cudaGetLastError());
+            return enqueue_energy(h, nullptr, 1, 0);
+        }
     } else if (!std::strcmp(key, "uniform_path")) {
         h->allow_uniform = value != 0;
         h->uniform_d = h->allow_uniform && h->all_d_equal;
@@ -541,6 +558,7 @@ int mc_get_option(mc_handle* h, const char* key, int64_t* value_host) {
     else if (!std::strcmp(key, "wave")) *value_host = h->pwave ? 1 : 0;
     else if (!std::strcmp(key, "form")) *value_host = h->form;
     else if (!std::strcmp(key, "form_auto")) *value_host = h->form_auto;
+    else if (!std::strcmp(key, "position_bits")) *value_host = h->p.pos_bits;
     else if (!std::strcmp(key, "uniform_path")) *value_host = h->uniform_d ? 1 : 0;
     else if (!std::strcmp(key, "stall_ms")) *value_host = (int64_t)(h->p.wait_limit_ns / 1000000ull);
     else if (!std::strcmp(key, "hist_slices")) *value_host = h->hist_slices;
@@ -599,8 +617,8 @@ int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers,
 }
 
 int mc_debug_peek(mc_handle* h, int32_t* out_host, int n) {
-    // n > 0: the first n scheduling words; n < 0: the first -n 32-bit words of the diagnostic counters
-    if (!h || !out_host || n == 0 || n > h->p.sy_n || -(int64_t)n * 4 > (int64_t)(kDbgWords * 8))
+    // n > 0: the first n scheduling words (live, then the snapshot); n < 0: the first -n 32-bit words of the diagnostic counters
+    if (!h || !out_host || n == 0 || n > 2 * h->p.sy_n || -(int64_t)n * 4 > (int64_t)(kDbgWords * 8))
         return fail(MC_EINVAL, "bad argument");
     cudaStream_t s2;
     CUDA_TRY(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));

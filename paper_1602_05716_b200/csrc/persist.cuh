@@ -32,7 +32,7 @@ constexpr int kHelpers = 6;
 #endif
 constexpr int kColsPerIter = MCB_COLS_PER_ITER;   // columns per iteration of the pair loop (2 pairs of rows x columns in flight per row)
 
-// scheduling state in global memory; zeroed by k_trial at the start of every sweep
+// scheduling state in global memory; zero at the start of every sweep (cleared by CTA 0 at the end of the one before)
 // (hot words 128 bytes apart, so that polling one does not slow down atomics on another)
 enum { kSyTicket = 0, kSyUTicket = 32, kSyGroups = 64, kSyChainSm = 96, kSyDTicket = 128, kSyAbort = 160, kSyTicketU = 192,
        kSyHdr = 256 };
@@ -46,7 +46,9 @@ struct PArgs {
     int nfar;         // number of FAR workers (0: do not round item counts to it)
     int mode;         // 0 normal; 1 throughput probe: no chain, every CTA runs QU items over all columns but the chunk's own;
                       // 2 watchdog test: the deciding warp never runs, so the sweep stalls
-    int* sy;          // [kSyHdr + 3 * nchunks]: header, far_done, diag_done, fix_done
+    int nsweeps;      // sweeps this launch runs (a1-a4 each), separated by grid-wide barriers
+    int* sy;          // [kSyHdr + 3 * nchunks]: header, far_done, diag_done, fix_done; all zero at launch and again at exit
+    int* gbar;        // grid barrier: [0] arrivals, [32] generation
     long long* dbg;   // [16] diagnostic cycle counters (see mc_debug_counters), may be null
 };
 
@@ -198,7 +200,7 @@ static __device__ __noinline__ int recheck_overlap_cg(const double2* xy, const d
 
 // Pair evaluation (Eq. 2; Alg. 2) in three forms, chosen by mc_init from the
 // geometry so that the per-trial dE stays within 1e-10 of its natural scale:
-//  GRAM  (20 FP64-pipe instructions + 2 MUFU; 22 if diameters differ)    cavity_R / d_min <= 64
+//  GRAM  (20 FP64-pipe instructions + 2 MUFU; 22 if diameters differ)    cavity_R / d_min <= 128
 //     r2o = |x_i|^2 + |x_j|^2 - 2 x_i.x_j       1 DADD + 3 DFMA   (|x_j|^2 is staged with the column)
 //     w   = 2 D.x_i + |D|^2 - 2 D.x_j           3 DFMA            (D = x~_i - x_i)
 //     r2n = r2o + w                             1 DADD
@@ -595,28 +597,37 @@ static __device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
                 Eu = __dadd_rn(Eu, __dadd_rn(__dadd_rn(s4[0], s4[1]), __dadd_rn(s4[2], s4[3])));
                 ovv = ovv || (((ho.ovnP[lane] & Ap) | (ho.ovoP[lane] & ~Ap)) != 0u);
             }
-            double Es = __fma_rn(lbq, Eu, lnu);
+            // Decisions of the 32 trials of this tile.  Trial l depends on the accept bits of the lanes j < l only
+            // (D(l, j) and the overlap bits are zero for j >= l), so the accept mask A is the unique fixed point of
+            //   A = F(A),  F(A)_l = [ no veto given A  and  ln u_l + l_B q_l (E0_l + sum_j A_j D(l, j)) < 0 ]
+            // and iterating F from any start fixes lane 0 in the first pass, lane 1 in the second, ...: at most 32
+            // passes, in practice one or two (the corrections D are tiny against |dE + ln u| except near a tie),
+            // each a masked sum instead of Alg. 4's 32 dependent steps.  Es < 0 is read off the
+            // sign bit (Es is never -0: ln u < 0 strictly and an exact cancellation gives +0).
             const unsigned ovo = ho.ovoD[lane], ovn = ho.ovnD[lane];
             const double* diag = ho.D + kTile * kTile;
-            bool veto = wallv || ovv;
-            unsigned A = 0u;
+            const double E0 = Eu;
+            const bool veto0 = wallv || ovv;
+            double Es = __fma_rn(lbq, E0, lnu);
+            unsigned A = __ballot_sync(0xffffffffu, !veto0 && (__double2hiint(Es) < 0));
+            bool hit = false;
+#pragma unroll 1
+            for (int pass = 0; pass <= kTile; ++pass) {
+                double s4[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-            for (int j = 0; j < kTile; ++j) {
-                const double dj = diag[j * kTile + lane];   // 0 for lanes <= j
-                const double djs = __dmul_rn(lbq, dj);
-                // Es < 0 read off the sign bit (Es is never -0: ln u < 0 strictly, and x + y = -0 needs x = y = -0)
-                const bool ok = !veto && (__double2hiint(Es) < 0);
-                const unsigned bal = __ballot_sync(0xffffffffu, ok);
-                const bool bit = ((bal >> j) & 1u) != 0u;
-                A |= (bit ? 1u : 0u) << j;
-                if (bit) {
-                    Es = __dadd_rn(Es, djs);
-                    Eu = __dadd_rn(Eu, dj);
+                for (int j = 0; j < kTile; ++j) {
+                    const double dj = diag[j * kTile + lane];   // 0 for lanes <= j
+                    s4[j & 3] = __dadd_rn(s4[j & 3], ((A >> j) & 1u) ? dj : 0.0);
                 }
-                const bool hit = (((bit ? ovn : ovo) >> j) & 1u) != 0u;  // bits >= lane are 0
-                veto = veto || hit;
-                ovv = ovv || hit;
+                Eu = __dadd_rn(E0, __dadd_rn(__dadd_rn(s4[0], s4[1]), __dadd_rn(s4[2], s4[3])));
+                Es = __fma_rn(lbq, Eu, lnu);
+                hit = ((ovn & A) | (ovo & ~A)) != 0u;             // bits >= lane are 0 in both words
+                const unsigned A1 = __ballot_sync(0xffffffffu, !veto0 && !hit && (__double2hiint(Es) < 0));
+                if (A1 == A) break;
+                A = A1;
             }
+            const bool veto = veto0 || hit;
+            ovv = ovv || hit;
             const bool acc = ((A >> lane) & 1u) != 0u;
             const bool tie = !veto && (fabs(Es) < 1e-8);
             ho.out_dE[lane] = __dmul_rn(lbq, Eu);
@@ -768,51 +779,48 @@ static __device__ __noinline__ void diag_item(const PArgs& a, PShared& sh, int c
                     sh.u.w.ch[warp], sh.u.w.ctz[warp]);
 }
 
-template <int ROWS, bool UNIFORM, int FORM>
-__global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    PShared& sh = *reinterpret_cast<PShared*>(smem_raw);
-    const int tid = threadIdx.x, warp = tid >> 5;
-    const Params& p = a.p;
-    const int C = a.C;
-    if (*(volatile int*)&p.st->stall) return;   // a stalled sweep invalidated the state: no-op (k_trial did nothing either)
-
-    if (tid == 0) {
-        for (int s = 0; s < kStages; ++s) {
-            mbar_init(&sh.full_bar[s], 1);
-            mbar_init(&sh.empty_bar[s], kPThreads / 32);
-        }
-        for (int s = 0; s < kRing; ++s) { mbar_init(&sh.ho_bar[s], 2); mbar_init(&sh.p_bar[s], 1); }
-        for (int s = 0; s < 2 * (kChunkMax / kTile); ++s) mbar_init(&sh.a_bar[0][0] + s, 1);
-        mbar_fence_init();
-        // the chain CTA gets its SM to itself: it publishes the SM it runs on, and the worker CTA
-        // that shares that SM retires at once
-        unsigned smid;
-        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        if (blockIdx.x == 0) {
-            st_release(a.sy + kSyChainSm, (int)smid + 1);
+// Grid-wide barrier between the phases of a launch (all CTAs are co-resident: cooperative launch).  Arrivals are
+// counted in gbar[0]; the last one resets the count and releases the others by bumping the generation gbar[32].
+// The acquire load (LDG.STRONG.GPU + CCTL.IVALL) also drops this SM's L1, so plain loads after the barrier see
+// what the other CTAs wrote before it.
+__device__ __forceinline__ void grid_barrier(const PArgs& a) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
+        int* cnt = a.gbar;
+        int* gen = a.gbar + 32;
+        const int g0 = ld_acquire(gen);          // read before arriving: nobody can bump it until this CTA has arrived
+        __threadfence();
+        if (atomicAdd(cnt, 1) == (int)gridDim.x - 1) {
+            *(volatile int*)cnt = 0;
+            __threadfence();
+            st_release(gen, g0 + 1);
         } else {
-            int v;
-            const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
             const unsigned long long t0 = global_ns();
-            for (unsigned it = 1; (v = ld_acquire(a.sy + kSyChainSm)) == 0; ++it) {
-                __nanosleep(100);
+            for (unsigned it = 1; ld_acquire(gen) == g0; ++it) {
+                __nanosleep(40);
                 if ((it & 1023u) == 0u) wd_check(wd, t0);
             }
-            sh.item[0] = (v == (int)smid + 1) ? 1 : 0;
         }
     }
     __syncthreads();
-    if (blockIdx.x == 0 && a.mode != 1) {
-        chain_cta(a, sh);
-        return;
-    }
-    if (sh.item[0] == 1 && a.mode != 1) return;
+}
 
+// a1 for the whole system, shared out over all threads of the grid; also clears the row accumulators
+static __device__ __noinline__ void trial_phase(const Params& p) {
+    const unsigned long long s = *(volatile unsigned long long*)&p.st->sweep;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < p.Np; i += gridDim.x * blockDim.x) trial_one(p, i, s);
+}
+
+// the worker loop of one sweep: pull items until every queue is exhausted
+template <int ROWS, bool UNIFORM, int FORM>
+__device__ __forceinline__ void worker_sweep(const PArgs& a, PShared& sh, unsigned& kring) {
+    const int tid = threadIdx.x, warp = tid >> 5;
+    const Params& p = a.p;
+    const int C = a.C;
     Cursors cur{{0, 0, -1}, {0, 0, -1}, {0, 0, -1}};
     if (a.dbg && blockIdx.x == 1 && tid == 0) a.dbg[16 + 3 * 300 + 40] = (long long)global_ns();
     const bool near = (int)blockIdx.x <= a.nnear;
-    unsigned kring = 0;
     for (;;) {
         __syncthreads();
         if (tid == 0) {
@@ -864,6 +872,92 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
                 const unsigned long long dt = (unsigned long long)(clock64() - t_item);
                 atomicAdd((unsigned long long*)a.dbg + 10 + (ty == kItemFarU ? kItemFarL : ty == kItemMid ? kItemFix : ty), dt);   // busy cycles: [11] diag [12] far [13] fix
                 if (near) atomicAdd((unsigned long long*)a.dbg + 14, dt);                              // [14] near workers
+            }
+        }
+    }
+}
+
+// One launch = a.nsweeps full sweeps.  Per sweep: trial generation by the whole grid (a1), grid barrier, the sweep
+// proper (chain CTA + workers, a2-a4), grid barrier, reset of the scheduling words.  mc_sweep(n) is therefore one
+// launch whatever n is (PAPER.md:85-91 launched one kernel per cycle and generated the random numbers on the host).
+template <int ROWS, bool UNIFORM, int FORM>
+__global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    PShared& sh = *reinterpret_cast<PShared*>(smem_raw);
+    const int tid = threadIdx.x;
+    const Params& p = a.p;
+    if (*(volatile int*)&p.st->stall) return;   // a stalled sweep invalidated the state: every later sweep is a no-op
+
+    auto init_chain_barriers = [&]() {
+        for (int s = 0; s < kRing; ++s) { mbar_init(&sh.ho_bar[s], 2); mbar_init(&sh.p_bar[s], 1); }
+        for (int s = 0; s < 2 * (kChunkMax / kTile); ++s) mbar_init(&sh.a_bar[0][0] + s, 1);
+    };
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(&sh.full_bar[s], 1);
+            mbar_init(&sh.empty_bar[s], kPThreads / 32);
+        }
+        init_chain_barriers();
+        mbar_fence_init();
+        // the chain CTA gets its SM to itself: it publishes the SM it runs on, and the worker CTA
+        // that shares that SM does no work in this launch (it only takes part in the grid barriers)
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        if (blockIdx.x == 0) {
+            st_release(a.sy + kSyChainSm, (int)smid + 1);
+        } else {
+            int v;
+            const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
+            const unsigned long long t0 = global_ns();
+            for (unsigned it = 1; (v = ld_acquire(a.sy + kSyChainSm)) == 0; ++it) {
+                __nanosleep(100);
+                if ((it & 1023u) == 0u) wd_check(wd, t0);
+            }
+            sh.item[3] = (v == (int)smid + 1) ? 1 : 0;
+        }
+    }
+    __syncthreads();
+    const bool is_chain = blockIdx.x == 0 && a.mode != 1;
+    const bool idle = blockIdx.x != 0 && sh.item[3] == 1 && a.mode != 1;
+
+    unsigned kring = 0;
+    for (int sw = 0; sw < a.nsweeps; ++sw) {
+        trial_phase(p);
+        grid_barrier(a);
+        if (is_chain) {
+            if (sw > 0) {      // the hand-off barriers start every sweep in phase 0
+                if (tid == 0) {
+                    for (int s = 0; s < 2 * kRing + 2 * (kChunkMax / kTile); ++s)
+                        asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&sh.ho_bar[0] + s)) : "memory");
+                    init_chain_barriers();
+                    mbar_fence_init();
+                }
+                __syncthreads();
+            }
+            chain_cta(a, sh);
+        } else if (!idle) {
+            worker_sweep<ROWS, UNIFORM, FORM>(a, sh, kring);
+        }
+        grid_barrier(a);
+        // everybody is done with the scheduling words: CTA 0 clears them for the next sweep (or the next launch);
+        // the election word stays until the launch ends.  The next reader is behind the next grid barrier.
+        if (blockIdx.x == 0) {
+            // the protocol's own invariant: every item of the plan ran
+            // exactly once -- each chunk's completion counters equal the item counts the plan gives for it
+            if (a.mode == 0) {
+                int bad = 0;
+                for (int c = tid; c < a.nchunks; c += kPThreads) {
+                    bad |= a.sy[kSyHdr + c] != far_items(p.Np, a.C, a.farcols, a.nfar, c);
+                    bad |= a.sy[kSyHdr + a.nchunks + c] != diag_items(chunk_rows(p.Np, a.C, c));
+                    bad |= a.sy[kSyHdr + 2 * a.nchunks + c] != urgent_items(a.C, c);
+                }
+                if (__syncthreads_or(bad) && tid == 0) p.st->sched_mismatch += 1;
+            }
+            // snapshot for mc_debug_peek, then clear
+            const bool last = sw + 1 == a.nsweeps;
+            for (int j = tid; j < p.sy_n; j += kPThreads) {
+                a.sy[p.sy_n + j] = a.sy[j];
+                if (last || j != kSyChainSm) a.sy[j] = 0;
             }
         }
     }

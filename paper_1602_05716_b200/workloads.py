@@ -66,7 +66,8 @@ class Workload:
         if "a" not in self._cache:
             q = np.concatenate([np.full(s.count, s.valence) for s in self.species]).astype(np.float64)
             d = np.concatenate([np.full(s.count, s.diameter) for s in self.species]).astype(np.float64)
-            pos = random_sequential_insertion(d, self.cavity_R, self.seed)
+            # (larger candidate batches for the million-ion system: fewer k-d tree rebuilds)
+            pos = random_sequential_insertion(d, self.cavity_R, self.seed, batch=8192 if self.N <= 300000 else 131072)
             if self.interleave:
                 perm = np.random.default_rng(self.seed + 7919).permutation(self.N)
                 pos, q, d = pos[:, perm], q[perm], d[perm]
@@ -164,8 +165,30 @@ CONFIGS = (
 HEADLINE = CONFIGS[3]
 
 
+def _paper_shaped() -> Workload:
+    """The paper's production system, in units of the ion diameter d = 7.5 A:
+    N = 1024 x 1024 ions of a 3:-1 electrolyte, ion radius 3.75 A, Bjerrum
+    length 7.117 A => l_B = 0.94893 d, bare Debye length 28.53 A = 3.804 d
+    => by Eq. 5 with sum n z^2 = 3 n_total: rho* = n_total d^3 = kappa^2 / (12 pi l_B) = 1.9317e-3, R = 506.1 d;
+    hard-wall sphere; trial cube of edge L/3 with L = 2R the size of the domain => max
+    displacement R/3.  g(r): 500 bins of 0.1 d to 50 d = 13 Debye lengths; centres at least that far from the wall
+    (the paper leaves out ions closer than 10 Debye lengths)."""
+    lB = 7.117 / 7.5
+    kappa = 7.5 / 28.53
+    rho = kappa * kappa / (12.0 * math.pi * lB)
+    N = 1024 * 1024
+    R = (3.0 * (N / rho) / (4.0 * math.pi)) ** (1.0 / 3.0)
+    return Workload("paper_3to1_n1048576", (Species(N // 4, +3.0, 1.0), Species(3 * N // 4, -1.0, 1.0)), rho, R / 3.0,
+                    3, bjerrum=lB, hist_bin_width=0.1, hist_nbins=500,
+                    note="paper-shaped production workload: N = 2^20, 3:-1, dilute, trial cube ~ L/3")
+
+
+PAPER_SHAPED = _paper_shaped()
+EXTRA = (PAPER_SHAPED,)
+
+
 def by_name(name: str) -> Workload:
-    for w in CONFIGS:
+    for w in CONFIGS + EXTRA:
         if w.name == name:
             return w
     raise KeyError(name)

@@ -83,3 +83,87 @@ def test_standard_error_of_a_correlated_series_matches_the_spread_of_independent
         means.append(x.mean()); ses.append(A.standard_error(x))
     assert abs(np.mean(ses) / np.std(means) - 1.0) < 0.15
     assert A.standard_error(np.ones(50)) == 0.0
+
+
+# ---------------------------------------------------------------------------------------------------
+# Eq. 5-8, 13-18 on synthetic Yukawa tails with known kappa_R, q^R, eps_R
+# ---------------------------------------------------------------------------------------------------
+def _yukawa_system(linear: bool):
+    """A 3:-1 electrolyte whose pair correlations are EXACTLY the dressed-ion far field (Eq. 7):
+    beta U_ab = q_a^R q_b^R (l_B eps/eps_R) exp(-kappa_R r) / r, with kappa_R^2 = 4 pi l_B sum_c n_c q_c q_c^R
+    (the relation that makes Eq. 12 reproduce Eq. 13; for a neutral binary mixture it is Eq. 8).
+    linear: g = 1 - beta U (then every identity of the chain holds exactly); else g = exp(-beta U)."""
+    lB, R = 0.949, 200.0
+    z = np.array([3.0, -1.0])
+    N = np.array([25000.0, 75000.0])
+    V = 4 * np.pi * R ** 3 / 3
+    n = N / V
+    zR = np.array([4.125, -0.884])                      # the paper's fitted values, as inputs here (PAPER.md:411)
+    eps_ratio = 1.07
+    kR = np.sqrt(4 * np.pi * lB * np.sum(n * z * zR))
+    bw, nb = 0.25, 400
+    r = bw * (np.arange(nb) + 0.5)
+    U = np.array([[zR[a] * zR[b] * (lB / eps_ratio) * np.exp(-kR * r) / r for b in range(2)] for a in range(2)])
+    g = 1.0 - U if linear else np.exp(-U)
+    return dict(lB=lB, R=R, z=z, N=N, n=n, zR=zR, eps_ratio=eps_ratio, kR=kR, r=r, U=U, g=g, bw=bw, nb=nb)
+
+
+def test_bare_kappa_is_the_pb_formula():
+    # 1:1, n_+ = n_- = n: kappa^2 = 8 pi l_B n (textbook Debye-Hueckel); config 1 of BASELINE: 1/kappa = 0.688 sigma
+    R = (3 * 512 / 0.1 / (4 * np.pi)) ** (1 / 3)
+    k = A.bare_kappa([256, 256], [1.0, -1.0], R, 1.68)
+    assert abs(k - np.sqrt(8 * np.pi * 1.68 * 0.05)) < 1e-12
+    assert abs(1 / k - 0.688) < 1e-3                     # SURVEY.md 8(d) table
+    # charge-asymmetric: every species weighs in with q^2
+    assert abs(A.bare_kappa([100, 300], [3.0, -1.0], 10.0, 1.0) ** 2
+               - 4 * np.pi * (100 * 9 + 300 * 1) / (4 * np.pi * 1000 / 3)) < 1e-12
+
+
+def test_tail_fit_recovers_kappa_R_exactly_on_a_yukawa_tail():
+    s = _yukawa_system(linear=True)
+    rho = A.charge_density(s["g"], s["N"], s["z"], s["R"])
+    # Eq. 13 with its sign: negative around the cation, positive around the anion
+    assert np.all(rho[0][20:120] < 0) and np.all(rho[1][20:120] > 0)
+    # window 5..30 sigma: beyond it the tail (< 1e-5 of the uniform background) drowns in the rounding of 1 - beta U
+    for b in range(2):
+        f = A.fit_kappa_R(s["r"], rho[b], 5.0, 30.0)
+        assert abs(f["kappa_R"] - s["kR"]) < 1e-8 * s["kR"]
+        assert f["sign"] == (-1.0 if b == 0 else 1.0)
+        # intercept of Eq. 14: log(kappa_R^2 |q^R| / (4 pi eps_R/eps))
+        want = np.log(s["kR"] ** 2 * abs(s["zR"][b]) / (4 * np.pi * s["eps_ratio"]))
+        assert abs(f["intercept"] - want) < 1e-7
+    # a wrong slope is seen: a tail that decays with another kappa gives that kappa
+    f = A.fit_kappa_R(s["r"], rho[0] * np.exp(-0.01 * s["r"]), 5.0, 30.0)
+    assert abs(f["kappa_R"] - (s["kR"] + 0.01)) < 1e-8
+
+
+def test_renormalized_valences_two_ways_permittivity_and_eq8_exact_on_linear_tails():
+    s = _yukawa_system(linear=True)
+    rho = A.charge_density(s["g"], s["N"], s["z"], s["R"])
+    U = s["U"]                                          # for g = 1 - U the PMF of Eq. 11 is not U; feed U itself
+    w = (5.0, 30.0)
+    qp = [A.renormalized_valence(s["r"], U[a, 0], rho[a], s["kR"], s["lB"], *w) for a in range(2)]   # Eq. 17a, both ways
+    qm = [A.renormalized_valence(s["r"], U[a, 1], rho[a], s["kR"], s["lB"], *w) for a in range(2)]   # Eq. 17b
+    assert np.allclose(qp, s["zR"][0], rtol=1e-8) and np.allclose(qm, s["zR"][1], rtol=1e-8)
+    e = [A.renormalized_permittivity(s["r"], rho[a], s["zR"][a], s["kR"], *w) for a in range(2)]     # Eq. 18, both ways
+    assert np.allclose(e, s["eps_ratio"], rtol=1e-8)
+    k0 = A.bare_kappa(s["N"], s["z"], s["R"], s["lB"])
+    lhs, rhs = A.dressed_ion_identity(s["kR"], k0, s["zR"][0], s["zR"][1], s["z"][0], s["z"][1])
+    assert abs(lhs - rhs) < 1e-12                       # Eq. 8 holds identically for this construction
+    assert lhs > 1.0                                    # 4.125, -0.884 vs 3, -1: kappa_R > kappa, as the paper finds (25.57 < 28.53 A)
+
+
+def test_whole_chain_from_histogram_counts_on_exponential_tails():
+    """Counts -> g -> U, rho -> kappa_R, q^R, eps_R: with g = exp(-beta U) the far-field values come back to the
+    accuracy of the linearisation (beta U ~ 1e-3 in the window)."""
+    s = _yukawa_system(linear=False)
+    shells = A.shell_volumes(s["bw"], s["nb"])
+    ncent = np.array([4000.0, 12000.0]) * 50            # centres accumulated over 50 samples
+    hist = np.array([[s["g"][a, b] * ncent[a] * s["n"][b] * shells for b in range(2)] for a in range(2)])
+    out = A.renormalized_parameters(hist, ncent, s["N"], s["z"], s["R"], s["bw"], s["lB"], 12.0, 30.0)
+    assert abs(out["kappa_R"] - s["kR"]) < 2e-3 * s["kR"]
+    assert np.allclose(out["qR_plus"], s["zR"][0], rtol=5e-3) and np.allclose(out["qR_minus"], s["zR"][1], rtol=5e-3)
+    assert np.allclose(out["epsR_over_eps"], s["eps_ratio"], rtol=1e-2)
+    lhs, rhs = out["eq8"]
+    assert abs(lhs - rhs) < 1e-2 * rhs
+    assert abs(out["kappa"] - A.bare_kappa(s["N"], s["z"], s["R"], s["lB"])) == 0.0

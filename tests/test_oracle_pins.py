@@ -421,3 +421,40 @@ def test_pair_hist_threaded_matches_serial():
     ha, na = a.pair_hist(0.05, 60, 0.7 * w.cavity_R)
     hb, nb_ = b.pair_hist(0.05, 60, 0.7 * w.cavity_R)
     assert np.array_equal(ha, hb) and np.array_equal(na, nb_) and ha.sum() > 0
+
+
+# ---- FP32-position variant -----------------------------------
+def test_fp32_position_mode_holds_only_fp32_values_and_rounds_the_trial_once_more():
+    from fractions import Fraction
+    w = W.scaled(W.CONFIGS[2], 300)
+    pos, q, d = w.arrays()
+    o = Oracle(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 9)
+    o.set_position_bits(32)
+    p0 = o.positions
+    assert np.array_equal(p0, pos.astype(np.float32).astype(np.float64))            # rounded to nearest at the switch
+    assert abs(o.stats()["E_running"] - o.energy()) < 1e-12 * abs(o.energy())         # running energy of the rounded state
+    o.sweep(1)
+    lg = o.trial_log()
+    # every proposed position = float32( correctly rounded fma(u - 1/2, 2 delta, x) ), checked with exact rationals
+    D = Fraction(2.0 * w.max_disp)
+    for i in (0, 1, 17, 150, 299):
+        A = philox4x32_10((i, 0, 0, 0), (9, 0)); B = philox4x32_10((i, 0, 0, 1), (9, 0))
+        u = [uniform_open01(A[0], A[1]), uniform_open01(A[2], A[3]), uniform_open01(B[0], B[1])]
+        for k in range(3):
+            # x_i at its turn: unchanged since the switch unless an earlier particle... no: only i moves x_i
+            exact = (Fraction(u[k]) - Fraction(1, 2)) * D + Fraction(p0[k, i])
+            want = float(np.float32(float(exact)))                                   # double rounding, as defined
+            assert lg["trial"][k, i] == want
+    p1 = o.positions
+    assert np.array_equal(p1, p1.astype(np.float32).astype(np.float64))              # still FP32 values after a sweep
+    assert (lg["flags"] & 1).sum() > 30
+    # the invariants hold in this mode as well (P5, P6)
+    o.sweep(20)
+    assert abs(o.stats()["E_running"] - o.energy()) < 1e-9 * abs(o.energy())
+    x = o.positions.T
+    r = np.linalg.norm(x[:, None] - x[None], axis=2) + np.eye(w.N) * 10
+    assert (r >= 0.5 * (d[:, None] + d[None, :]) * (1 - 1e-15)).all()
+    # and it is a different chain from the FP64 one
+    o64 = Oracle(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 9)
+    o64.sweep(21)
+    assert not np.array_equal(o64.positions, o.positions)
