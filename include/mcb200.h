@@ -80,6 +80,13 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
  * mc_sweep(a); mc_sweep(b) is bit-identical to mc_sweep(a+b).   PAPER.md:43-73, Alg. 1-5. */
 int mc_sweep(mc_handle* h, int64_t n);
 
+/* The same n sweeps -- the same chain, bit for bit in the accept/reject sequence -- by the paper's COMPARISON
+ * code, the "parallel reduction scheme" of PAPER.md:278-282: one kernel launch per trial (N per sweep), the
+ * N-1 pair terms spread over blocks of 1024 threads, warp-shuffle reductions, atomic sub-totals, a counter of
+ * completed blocks, the last block decides.  Exists to reproduce the paper's comparison (Fig. 8-10), not for
+ * speed.  Enqueued, no host sync.  mc_sweep and mc_sweep_reduction may be mixed freely. */
+int mc_sweep_reduction(mc_handle* h, int64_t n);
+
 /* From-scratch total energy l_B sum_{i<j} q_i q_j / r_ij in k_B T (monitored
  * during warm-up).  Synchronises. */
 int mc_energy(mc_handle* h, double* E_host);
@@ -177,12 +184,16 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
  *   "uniform_path" 0|1     allow the equal-diameter specialisation (default 1)
  *   "stall_ms"     0..3600000  watchdog limit per wait of the sweep kernel in ms (default 2000; 0 = none;
  *                          raise it under a profiler, a sanitizer or GPU time-slicing)
+ *   "max_ctas"     0..4096 upper limit on the CTAs of the sweep kernel (0 = two per SM, the default for large
+ *                          systems; small systems synchronise faster on a smaller grid)
+ *   "energy_rows"  4|6|8   rows per thread of the from-scratch energy kernel
  *   "hist_slices"  1..64   column slices of the pair-histogram kernel (default 32)
  *   "debug"        0|1     collect the counters of mc_debug_counters (default 0)
  *   "probe"        0|1|2   needs debug = 1.  1: the next sweeps run the worker loop alone over all columns
  *                          (throughput probe); their results are meaningless and the sweep index stands still.
  *                          2: the deciding warp never runs, so the next sweep stalls (tests MC_ESTALL)
- * mc_get_option reads a setting back ("form_auto": the form the geometry allows). */
+ * mc_get_option reads a setting back ("form_auto": the form the geometry allows; "grid": CTAs of the
+ * last k_sweep launch, 2 per SM). */
 int mc_set_option(mc_handle* h, const char* key, int64_t value);
 int mc_get_option(mc_handle* h, const char* key, int64_t* value_host);
 

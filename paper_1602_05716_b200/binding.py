@@ -20,7 +20,7 @@ _CODES = {-1: "MC_EINVAL", -2: "MC_EOVERLAP", -3: "MC_EOUTSIDE", -4: "MC_ENOSPAC
 
 EXPORTS = (
     "mc_workspace_bytes", "mc_init", "mc_sweep", "mc_energy", "mc_energy_dev", "mc_pair_hist", "mc_sweep_host",
-    "mc_sweep_timed",
+    "mc_sweep_timed", "mc_sweep_reduction",
     "mc_get_positions", "mc_set_positions", "mc_set_state", "mc_get_sweep_index", "mc_set_sweep_index", "mc_get_stats",
     "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option", "mc_get_option",
     "mc_debug_counters", "mc_debug_peek", "mc_plan_check",
@@ -55,6 +55,7 @@ def load_library() -> C.CDLL:
     lib.mc_workspace_bytes.argtypes = [i64]; lib.mc_workspace_bytes.restype = C.c_size_t
     lib.mc_init.argtypes = [C.POINTER(vp), i64, vp, vp, vp, dbl, dbl, dbl, u64, vp, C.c_size_t, vp, C.c_int]
     lib.mc_sweep.argtypes = [vp, i64]
+    lib.mc_sweep_reduction.argtypes = [vp, i64]
     lib.mc_energy.argtypes = [vp, C.POINTER(dbl)]
     lib.mc_energy_dev.argtypes = [vp, vp]
     lib.mc_sweep_timed.argtypes = [vp, i64, C.POINTER(dbl)]
@@ -161,6 +162,10 @@ class MCSystem:
         _check(self._lib.mc_sweep(self._h, int(n)))
 
     sweep = mc_sweep
+
+    def mc_sweep_reduction(self, n: int = 1):
+        """The paper's comparison code: the same chain, one kernel launch per trial."""
+        _check(self._lib.mc_sweep_reduction(self._h, int(n)))
 
     def mc_energy(self) -> float:
         e = C.c_double()

@@ -1,6 +1,6 @@
 // aux_kernels.cuh -- the kernels of libmcb200 around the sweep (sm_100a): packing and accessors, from-scratch energy (a5), pair histograms (a6), the FP64 peak probe.  Included by mcb200.cu only.
 #pragma once
-#include "kernels.cuh"
+#include "persist.cuh"   // the scheduling words (kSy*) the comparison kernel borrows
 
 namespace mcb {
 
@@ -94,17 +94,19 @@ __global__ void k_check_particles(Params p, const double* d) {
 // j > i per pair.  Every CTA reduces its rows in a fixed order and writes one partial; k_energy_reduce
 // adds the partials in index order.
 // ------------------------------------------------------------------------------------------
-constexpr int kERows = 4, kEBlock = 256 * kERows, kETile = 256;
+constexpr int kETile = 256;
 
-__host__ __device__ inline int energy_units(int Np) {
-    const int nrb = (Np + kEBlock - 1) / kEBlock;
+__host__ __device__ inline int energy_units(int Np, int rows = 4) {
+    const int eblock = 256 * rows;
+    const int nrb = (Np + eblock - 1) / eblock;
     int n = 0;
-    for (int rb = 0; rb < nrb; ++rb) n += ((Np - rb * kEBlock) + kETile - 1) / kETile;
+    for (int rb = 0; rb < nrb; ++rb) n += ((Np - rb * eblock) + kETile - 1) / kETile;
     return n;
 }
 
-template <bool CHECK, bool GRAM>
+template <bool CHECK, bool GRAM, int kERows>
 __global__ void __launch_bounds__(256, 2) k_energy(Params p, double* part) {
+    constexpr int kEBlock = 256 * kERows;
     __shared__ double2 sxy[kETile], szq[kETile];
     __shared__ double sh[kETile], sn[kETile];
     __shared__ double red[8];
@@ -427,6 +429,91 @@ __global__ void __launch_bounds__(256) k_hist(Params p, const int* list, const i
         const unsigned v = shist[b];
         if (v) atomicAdd(&hist[b], (unsigned long long)v);
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// The paper's comparison code ("GPU code with parallel reduction
+// scheme"): ONE KERNEL PER TRIAL.  The N-1 pair terms of trial i are spread over N threads in blocks of 1024
+// (the thread of the selected particle stays idle), summed inside a block with warp shuffles, through shared
+// memory, and with warp shuffles again; every block adds its sub-total to global memory atomically and then
+// increases a global counter of completed blocks; the block that completes the count decides the move and
+// updates the particle.  Kept for the comparison the paper makes, not for speed: N launches per sweep.
+// Sub-totals go through the same fixed-point accumulators as the sweep kernel's (accum_row), so the result
+// does not depend on the order in which the blocks arrive.  Both distances are formed from rounded
+// differences (reading G11), whatever the geometry.
+// ------------------------------------------------------------------------------------------
+constexpr int kRedThreads = 1024;
+__global__ void __launch_bounds__(kRedThreads) k_reduction_trial(Params p, int i) {
+    __shared__ double s_t[4];
+    __shared__ int s_wall, s_last;
+    __shared__ double wsum[kRedThreads / 32];
+    __shared__ int wov[kRedThreads / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const double2 xyi = p.xy[i];
+    const double zi = p.zq[i].x, hi = p.hh[i];
+    if (tid == 0) {
+        const Trial t = trial_compute(p, i, p.st->sweep, xyi, zi);
+        s_t[0] = t.x; s_t[1] = t.y; s_t[2] = t.z; s_t[3] = t.lnu;
+        s_wall = t.wall;
+    }
+    __syncthreads();
+    const double tx = s_t[0], ty = s_t[1], tz = s_t[2];
+    const int j = blockIdx.x * kRedThreads + tid;
+    double term = 0.0;
+    int ov = 0;
+    if (j < p.N && j != i) {
+        const double2 a = p.xy[j], b = p.zq[j];
+        const double sij = __dadd_rn(hi, p.hh[j]);
+        const double r2o = dist2(__dadd_rn(xyi.x, -a.x), __dadd_rn(xyi.y, -a.y), __dadd_rn(zi, -b.x));
+        const double r2n = dist2(__dadd_rn(tx, -a.x), __dadd_rn(ty, -a.y), __dadd_rn(tz, -b.x));
+        ov = (r2n < __dmul_rn(sij, sij)) ? 1 : 0;
+        if (!ov) term = __dmul_rn(b.y, __dadd_rn(rsqrt_fast(r2n), -rsqrt_fast(r2o)));   // G14: an overlapping trial's dE is never used
+    }
+    // reduction within the block: warp shuffles, shared memory, warp shuffles again
+    term = warp_sum(term);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ov += __shfl_xor_sync(0xffffffffu, ov, o);
+    if (lane == 0) { wsum[warp] = term; wov[warp] = ov; }
+    __syncthreads();
+    if (warp == 0) {
+        term = warp_sum(wsum[lane]);
+        ov = wov[lane];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ov += __shfl_xor_sync(0xffffffffu, ov, o);
+        if (lane == 0) {
+            accum_row(p, i, term, ov);                       // sub-total into global memory, atomically
+            __threadfence();
+            s_last = atomicAdd(p.sy + kSyTicket, 1) == (int)gridDim.x - 1;   // the counter of completed blocks
+        }
+    }
+    __syncthreads();
+    if (!s_last || tid != 0) return;
+    // the last block decides (Eq. 1 in log form, readings G3, G4) and updates the selected particle
+    __threadfence();
+    const double E = accum_value(__ldcg(p.S1 + i), __ldcg(p.S2 + i));
+    const bool ovv = __ldcg(p.ovc + i) > 0, wallv = s_wall != 0;
+    const double lbq = p.lbq[i];
+    const double Es = __fma_rn(lbq, E, s_t[3]);
+    const bool acc = !ovv && !wallv && (__double2hiint(Es) < 0);
+    const bool tie = !ovv && !wallv && (fabs(Es) < 1e-8);
+    const double dE = __dmul_rn(lbq, E);
+    DevState* st = p.st;
+    if (acc) {
+        p.xy[i] = make_double2(tx, ty);
+        p.zq[i].x = tz;
+        p.nn[i] = dist2(tx, ty, tz);
+        st->E_run = __dadd_rn(st->E_run, dE);
+        st->accepted += 1ull;
+    }
+    st->veto_overlap += ovv ? 1ull : 0ull;
+    st->veto_wall += wallv ? 1ull : 0ull;
+    st->near_ties += tie ? 1ull : 0ull;
+    p.log_dE[i] = dE;
+    p.log_flags[i] = (unsigned char)((acc ? kFlagAccept : 0u) | (ovv ? kFlagOverlap : 0u) | (wallv ? kFlagWall : 0u) |
+                                     (tie ? kFlagNearTie : 0u));
+    p.S1[i] = 0ll; p.S2[i] = 0ll; p.ovc[i] = 0;
+    p.sy[kSyTicket] = 0;
+    if (i == p.N - 1) st->sweep += 1ull;
 }
 
 // ------------------------------------------------------------------------------------------

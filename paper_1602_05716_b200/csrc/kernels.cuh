@@ -51,14 +51,11 @@ __device__ __forceinline__ double accum_value(long long s1, long long s2) {
 // (G2), Philox keyed by (seed; particle, sweep, tag) (G9), hard wall (G6).  Also clears the row's
 // accumulators.  Runs inside the sweep kernel (persist.cuh: trial_phase), all threads of the grid.
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ void trial_one(const Params& p, int i, unsigned long long s) {
-    p.S1[i] = 0ll; p.S2[i] = 0ll; p.ovc[i] = 0;
-    const double2 xy = p.xy[i];
-    const double2 zq = p.zq[i];
-    if (i >= p.N) {  // ghost padding: never moves
-        p.txy[i] = xy; p.tz[i] = zq.x; p.lnu[i] = 0.0; p.wall[i] = (unsigned char)kFlagWall;
-        return;
-    }
+struct Trial {
+    double x, y, z, lnu;
+    unsigned char wall;
+};
+__device__ __forceinline__ Trial trial_compute(const Params& p, int i, unsigned long long s, double2 xy, double zi) {
     const uint32_t k0 = (uint32_t)p.seed, k1 = (uint32_t)(p.seed >> 32);
     uint32_t A[4], B[4];
     philox4x32_10((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, k0, k1, A);
@@ -68,18 +65,32 @@ __device__ __forceinline__ void trial_one(const Params& p, int i, unsigned long 
     const double uz = uniform_open01(B[0], B[1]);
     const double ua = uniform_open01(B[2], B[3]);
     const double D = __dmul_rn(2.0, p.max_disp);
-    double tx = __fma_rn(__dadd_rn(ux, -0.5), D, xy.x);
-    double ty = __fma_rn(__dadd_rn(uy, -0.5), D, xy.y);
-    double tz = __fma_rn(__dadd_rn(uz, -0.5), D, zq.x);
+    Trial t;
+    t.x = __fma_rn(__dadd_rn(ux, -0.5), D, xy.x);
+    t.y = __fma_rn(__dadd_rn(uy, -0.5), D, xy.y);
+    t.z = __fma_rn(__dadd_rn(uz, -0.5), D, zi);
     if (p.pos_bits == 32) {   // the proposed position is stored as FP32: one more rounding, to nearest
-        tx = (double)__double2float_rn(tx); ty = (double)__double2float_rn(ty); tz = (double)__double2float_rn(tz);
+        t.x = (double)__double2float_rn(t.x); t.y = (double)__double2float_rn(t.y); t.z = (double)__double2float_rn(t.z);
     }
     const double a = __dadd_rn(p.R, -p.hh[i]);
-    const double rr = dist2(tx, ty, tz);
-    p.txy[i] = make_double2(tx, ty);
-    p.tz[i] = tz;
-    p.lnu[i] = log(ua);
-    p.wall[i] = (rr > __dmul_rn(a, a)) ? (unsigned char)kFlagWall : (unsigned char)0;
+    const double rr = dist2(t.x, t.y, t.z);
+    t.lnu = log(ua);
+    t.wall = (rr > __dmul_rn(a, a)) ? (unsigned char)kFlagWall : (unsigned char)0;
+    return t;
+}
+__device__ __forceinline__ void trial_one(const Params& p, int i, unsigned long long s) {
+    p.S1[i] = 0ll; p.S2[i] = 0ll; p.ovc[i] = 0;
+    const double2 xy = p.xy[i];
+    const double2 zq = p.zq[i];
+    if (i >= p.N) {  // ghost padding: never moves
+        p.txy[i] = xy; p.tz[i] = zq.x; p.lnu[i] = 0.0; p.wall[i] = (unsigned char)kFlagWall;
+        return;
+    }
+    const Trial t = trial_compute(p, i, s, xy, zq.x);
+    p.txy[i] = make_double2(t.x, t.y);
+    p.tz[i] = t.z;
+    p.lnu[i] = t.lnu;
+    p.wall[i] = t.wall;
 }
 
 // ------------------------------------------------------------------------------------------

@@ -80,11 +80,13 @@ struct mc_handle {
     int num_sms = 148;
     int prows = 4;           // rows per consumer thread of the sweep kernel (chunk = 256 * prows)
     int pfarcols = 256;      // columns per FAR item of the sweep kernel
+    int erows = 4;           // rows per thread of k_energy (Gram form)
     int hist_slices = kHistSlices;   // column slices (grid.y) of k_hist
     int pmode = 0;           // 1: throughput probe (diagnostic, needs "debug"; the sweep's results are meaningless)
     bool pwave = true;       // round the FAR items of a chunk to a multiple of the FAR workers
     int pnear = 4;           // worker CTAs of the sweep kernel that serve urgent and DIAG items only
     bool debug = false;      // collect the cycle counters of mc_debug_counters
+    int max_ctas = 0;        // upper limit on the CTAs of the sweep kernel (0: two per SM); small systems synchronise faster on a smaller grid
     int pgrid = 0;           // CTAs of the sweep kernel
     int pgrid_key = -1;      // (form, rows, uniform) the grid was sized and the kernel configured for
     bool uniform_d = false;  // all diameters equal: s_ij^2 is one constant
@@ -121,6 +123,7 @@ int launch_sweep(mc_handle* h, cudaStream_t s, int nsweeps) {
         if (e != cudaSuccess) return fail(MC_ECUDA, std::string("k_sweep configuration: ") + cudaGetErrorString(e));
         if (occ < 1) return fail(MC_ECUDA, "k_sweep does not fit on an SM");
         h->pgrid = std::min(occ, 2) * h->num_sms;
+        if (h->max_ctas > 0) h->pgrid = std::max(8, std::min(h->pgrid, h->max_ctas));
         h->pgrid_key = key;
     }
     PArgs& a = L.args;
@@ -154,11 +157,14 @@ int reset_scheduling(mc_handle* h) {
 
 int enqueue_energy(mc_handle* h, double* out_dev, int set_running, int check_overlap) {
     const Params& p = h->p;
-    const int units = energy_units(p.Np);
     const bool gram = h->form_auto == kFormGram;
-    if (check_overlap) k_energy<true, false><<<units, 256, 0, h->stream>>>(p, h->epart);
-    else if (gram) k_energy<false, true><<<units, 256, 0, h->stream>>>(p, h->epart);
-    else k_energy<false, false><<<units, 256, 0, h->stream>>>(p, h->epart);
+    const int rows = (check_overlap || !gram) ? 4 : h->erows;
+    const int units = energy_units(p.Np, rows);
+    if (check_overlap) k_energy<true, false, 4><<<units, 256, 0, h->stream>>>(p, h->epart);
+    else if (!gram) k_energy<false, false, 4><<<units, 256, 0, h->stream>>>(p, h->epart);
+    else if (rows == 8) k_energy<false, true, 8><<<units, 256, 0, h->stream>>>(p, h->epart);
+    else if (rows == 6) k_energy<false, true, 6><<<units, 256, 0, h->stream>>>(p, h->epart);
+    else k_energy<false, true, 4><<<units, 256, 0, h->stream>>>(p, h->epart);
     k_energy_reduce<<<1, 32, 0, h->stream>>>(p, h->epart, units, out_dev, set_running);
     h->launches += 2;
     CUDA_TRY(cudaGetLastError());
@@ -295,6 +301,22 @@ int mc_sweep(mc_handle* h, int64_t n) {
         if (rc != MC_OK) return rc;
         h->launches += 1;
         n -= m;
+    }
+    return MC_OK;
+}
+
+int mc_sweep_reduction(mc_handle* h, int64_t n) {
+    if (!h || n < 0) return fail(MC_EINVAL, "bad handle or n < 0");
+    const Params& p = h->p;
+    // the accumulators of the selected particle must be clean (k_sweep leaves its last sweep's sums in them)
+    CUDA_TRY(cudaMemsetAsync(p.S1, 0, (size_t)p.Np * 8, h->stream));
+    CUDA_TRY(cudaMemsetAsync(p.S2, 0, (size_t)p.Np * 8, h->stream));
+    CUDA_TRY(cudaMemsetAsync(p.ovc, 0, (size_t)p.Np * 4, h->stream));
+    const int blocks = (p.N + kRedThreads - 1) / kRedThreads;
+    for (int64_t s = 0; s < n; ++s) {
+        for (int i = 0; i < p.N; ++i) k_reduction_trial<<<blocks, kRedThreads, 0, h->stream>>>(p, i);
+        h->launches += (uint64_t)p.N;
+        CUDA_TRY(cudaGetLastError());
     }
     return MC_OK;
 }
@@ -511,6 +533,10 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     } else if (!std::strcmp(key, "pnear")) {
         if (value < 0 || value > 128) return fail(MC_EINVAL, "pnear must be in 0..128");
         h->pnear = (int)value;
+    } else if (!std::strcmp(key, "max_ctas")) {
+        if (value < 0 || value > 4096) return fail(MC_EINVAL, "max_ctas must be in 0..4096 (0: two per SM)");
+        h->max_ctas = (int)value;
+        h->pgrid_key = -1;
     } else if (!std::strcmp(key, "wave")) {
         h->pwave = value != 0;
     } else if (!std::strcmp(key, "form")) {
@@ -534,6 +560,9 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     } else if (!std::strcmp(key, "stall_ms")) {
         if (value < 0 || value > 3600000) return fail(MC_EINVAL, "stall_ms must be in 0..3600000 (0: no limit)");
         h->p.wait_limit_ns = (unsigned long long)value * 1000000ull;
+    } else if (!std::strcmp(key, "energy_rows")) {
+        if (value != 4 && value != 6 && value != 8) return fail(MC_EINVAL, "energy_rows must be 4, 6 or 8");
+        h->erows = (int)value;
     } else if (!std::strcmp(key, "hist_slices")) {
         if (value < 1 || value > 64) return fail(MC_EINVAL, "hist_slices must be in 1..64");
         h->hist_slices = (int)value;
@@ -556,14 +585,17 @@ int mc_get_option(mc_handle* h, const char* key, int64_t* value_host) {
     else if (!std::strcmp(key, "far_cols")) *value_host = h->pfarcols;
     else if (!std::strcmp(key, "pnear")) *value_host = h->pnear;
     else if (!std::strcmp(key, "wave")) *value_host = h->pwave ? 1 : 0;
+    else if (!std::strcmp(key, "max_ctas")) *value_host = h->max_ctas;
     else if (!std::strcmp(key, "form")) *value_host = h->form;
     else if (!std::strcmp(key, "form_auto")) *value_host = h->form_auto;
     else if (!std::strcmp(key, "position_bits")) *value_host = h->p.pos_bits;
     else if (!std::strcmp(key, "uniform_path")) *value_host = h->uniform_d ? 1 : 0;
     else if (!std::strcmp(key, "stall_ms")) *value_host = (int64_t)(h->p.wait_limit_ns / 1000000ull);
     else if (!std::strcmp(key, "hist_slices")) *value_host = h->hist_slices;
+    else if (!std::strcmp(key, "energy_rows")) *value_host = h->erows;
     else if (!std::strcmp(key, "debug")) *value_host = h->debug ? 1 : 0;
     else if (!std::strcmp(key, "probe")) *value_host = h->pmode;
+    else if (!std::strcmp(key, "grid")) *value_host = h->pgrid;
     else return fail(MC_EINVAL, std::string("unknown option ") + key);
     return MC_OK;
 }

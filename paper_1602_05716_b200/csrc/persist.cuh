@@ -116,6 +116,15 @@ static __device__ __noinline__ void wd_check(const Watch& w, unsigned long long 
     }
     asm volatile("exit;");
 }
+// the same test without the exit: true if the kernel is being abandoned (raises the flags itself when the limit has passed)
+static __device__ __noinline__ bool wd_poll(const Watch& w, unsigned long long t0) {
+    if (*(volatile int*)(w.sy + kSyAbort) != 0) return true;
+    if (w.limit == 0ull || global_ns() - t0 < w.limit) return false;
+    *(volatile int*)(w.sy + kSyAbort) = 1;
+    *(volatile int*)(&w.st->stall) = 1;
+    __threadfence();
+    return true;
+}
 __device__ __forceinline__ void spin_until_ge(const Watch& w, const int* p, int v) {
     if (ld_acquire(p) >= v) return;
     const unsigned long long t0 = global_ns();
@@ -133,7 +142,7 @@ __device__ __forceinline__ void mbar_wait_wd(const Watch& w, uint64_t* bar, uint
 
 // shared memory of one CTA: workers use the column ring, the chain CTA the hand-off ring
 struct HandOff {
-    double D[2 * kTile * kTile];   // blocks (t, t-1) and (t, t), [jj][lane] each
+    double D[3 * kTile * kTile];   // blocks (t, t-2), (t, t-1) and (t, t), [jj][lane] each (contiguous in Dblk)
     double E[kTile], lbq[kTile], lnu[kTile];
     double2 txy[kTile];
     double tz[kTile];
@@ -153,7 +162,8 @@ struct __align__(128) PShared {
         HandOff ho[kRing];
     } u;
     uint64_t full_bar[kStages], empty_bar[kStages];
-    uint64_t ho_bar[kRing];               // tile handed over (2 helper arrivals + bulk-copy bytes)
+    uint64_t ho_bar[kRing];               // tile handed over by its helper
+    uint64_t d_bar[kRing];                // the tile's three D blocks have landed in the slot (bulk-copy bytes)
     uint64_t p_bar[kRing];                // publisher done with the slot
     uint64_t a_bar[2][kChunkMax / kTile]; // accept mask of tile t of a chunk (by chunk parity) published
     unsigned sA[2][kChunkMax / kTile];
@@ -423,17 +433,18 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
         // the slot is free once the publisher is done with tile gt - kRing
         if (gt >= kRing) mbar_wait_wd(wd, &sh.p_bar[slot], (unsigned)(gt / kRing - 1) & 1u);
         if (lane == 0) {
-            const double* src = B.Dblk + (size_t)blk_index(t, t > 0 ? t - 1 : 0) * (kTile * kTile);
-            const uint32_t bytes = (t > 0 ? 2u : 1u) * kTile * kTile * 8u;
+            const int nb = min(t, 2) + 1;          // blocks (t, t-2), (t, t-1), (t, t): contiguous in Dblk
+            const double* src = B.Dblk + (size_t)blk_index(t, t + 1 - nb) * (kTile * kTile);
+            const uint32_t bytes = (uint32_t)nb * kTile * kTile * 8u;
             fence_proxy_async();
-            mbar_arrive_expect_tx(&sh.ho_bar[slot], bytes);
-            bulk_g2s(t > 0 ? ho.D : ho.D + kTile * kTile, src, bytes, &sh.ho_bar[slot]);
+            mbar_arrive_expect_tx(&sh.d_bar[slot], bytes);
+            bulk_g2s(ho.D + (3 - nb) * kTile * kTile, src, bytes, &sh.d_bar[slot]);
         }
         staged = true;
     };
 
-    // corrections of the column tiles s <= t - 2, as their accept masks appear
-    for (int s = 0; s + 2 <= t; ++s) {
+    // corrections of the column tiles s <= t - 3, as their accept masks appear (masked loads from L2)
+    for (int s = 0; s + 3 <= t; ++s) {
         if (!staged && s + kRing >= t) stage_blocks();
         mbar_wait_wd(wd, &sh.a_bar[c & 1][s], apar);
         const unsigned A = sh.sA[c & 1][s];
@@ -449,6 +460,24 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
         if (((on & A) | (oo & ~A)) != 0u) veto |= kFlagOverlap;
     }
     if (!staged) stage_blocks();
+    if (t >= 2) {
+        // column tile t - 2, decided one tile ago: its block is already in the slot, so that only shared-memory
+        // latency lies between the mask and the hand-over
+        const int s = t - 2;
+        const unsigned on = __ldcg(B.OVnew + (size_t)r * W + s), oo = __ldcg(B.OVold + (size_t)r * W + s);
+        mbar_wait_wd(wd, &sh.d_bar[slot], (unsigned)(gt / kRing) & 1u);
+        double v[kTile];
+#pragma unroll
+        for (int jj = 0; jj < kTile; ++jj) v[jj] = ho.D[jj * kTile + lane];
+        mbar_wait_wd(wd, &sh.a_bar[c & 1][s], apar);
+        const unsigned A = sh.sA[c & 1][s];
+        double s8[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+        for (int jj = 0; jj < kTile; ++jj) s8[jj & 7] = __dadd_rn(s8[jj & 7], ((A >> jj) & 1u) ? v[jj] : 0.0);
+        E = __dadd_rn(E, __dadd_rn(__dadd_rn(__dadd_rn(s8[0], s8[1]), __dadd_rn(s8[2], s8[3])),
+                                  __dadd_rn(__dadd_rn(s8[4], s8[5]), __dadd_rn(s8[6], s8[7]))));
+        if (((on & A) | (oo & ~A)) != 0u) veto |= kFlagOverlap;
+    }
 
     ho.E[lane] = E; ho.lbq[lane] = lbq; ho.lnu[lane] = lnu;
     ho.txy[lane] = txy; ho.tz[lane] = tz;
@@ -478,9 +507,11 @@ __device__ __forceinline__ void chain_publisher(const PArgs& a, PShared& sh) {
             const int i = row0 + t * kTile + lane;
             const unsigned fl = ho.out_flags[lane];
             const double dE = ho.out_dE[lane];
+            const double2 t2 = ho.txy[lane];
+            const double tz = ho.tz[lane];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sh.p_bar[slot]);      // the slot is free for tile gt + kRing before the global stores below
             if (fl & kFlagAccept) {
-                const double2 t2 = ho.txy[lane];
-                const double tz = ho.tz[lane];
                 p.xy[i] = t2;
                 p.zq[i].x = tz;
                 p.nn[i] = dist2(t2.x, t2.y, tz);
@@ -496,7 +527,6 @@ __device__ __forceinline__ void chain_publisher(const PArgs& a, PShared& sh) {
             }
             __syncwarp();
             if (lane == 0) {
-                mbar_arrive(&sh.p_bar[slot]);
                 const int rows_done = (t + 1) * kTile;
                 if (rows_done % kGroup == 0 || t + 1 == nt) {
                     __threadfence();
@@ -551,14 +581,14 @@ static __device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
         for (int c = 0; c < a.nchunks; ++c) {
             const int row0 = c * C, nrows = chunk_rows(p.Np, C, c), nt = nrows / kTile;
             if (h >= nt) continue;
-            if (lane == 0) {
+            {   // every lane polls (one broadcast load): the warp waits, and gives up, as a whole
                 const long long t0 = clock64();
                 spin_until_ge(wd, sy_far_done(a) + c, far_items(p.Np, C, a.farcols, a.nfar, c));
                 const long long t1 = clock64();
                 spin_until_ge(wd, sy_diag_done(a) + c, diag_items(nrows));
                 const long long t2 = clock64();
                 if (c > 0) spin_until_ge(wd, sy_fix_done(a) + c, urgent_items(C, c));
-                if (h == 0 && a.dbg) {
+                if (h == 0 && lane == 0 && a.dbg) {
                     a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t2; a.dbg[15] += t2 - t1;
                     if (c < 300) a.dbg[16 + 3 * c] = (long long)global_ns();   // inputs of chunk c complete
                 }
@@ -583,18 +613,30 @@ static __device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
             mbar_wait_wd(wd, &sh.ho_bar[slot], (unsigned)(gt / kRing) & 1u);
             if (t == 0) w_first += clock64() - tw; else w_other += clock64() - tw;
             if (t == 0 && lane == 0 && a.dbg && c < 300) a.dbg[16 + 3 * c + 1] = (long long)global_ns();   // chain starts chunk c
+            mbar_wait_wd(wd, &sh.d_bar[slot], (unsigned)(gt / kRing) & 1u);   // (complete long ago; makes the copy visible here)
             HandOff& ho = sh.u.ho[slot];
+            // the tile's two nearest blocks, one row each per lane, into registers: every pass below is then pure arithmetic
+            double dp[kTile], dd[kTile];
+            {
+                const double* prev = ho.D + kTile * kTile;
+                const double* diag = ho.D + 2 * kTile * kTile;
+#pragma unroll
+                for (int j = 0; j < kTile; ++j) { dp[j] = prev[j * kTile + lane]; dd[j] = diag[j * kTile + lane]; }   // dd: 0 for lanes <= j
+            }
             const double lbq = ho.lbq[lane], lnu = ho.lnu[lane];
             double Eu = ho.E[lane];
             const unsigned vflags = ho.veto[lane];
             const bool wallv = (vflags & kFlagWall) != 0u;
             bool ovv = (vflags & kFlagOverlap) != 0u;
-            if (t > 0) {  // corrections of the tile just resolved: block (t, t-1)
-                double s4[4] = {0.0, 0.0, 0.0, 0.0};
+            auto masked_sum = [](const double (&d)[kTile], unsigned A) {
+                double s8[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-                for (int jj = 0; jj < kTile; ++jj)
-                    if ((Ap >> jj) & 1u) s4[jj & 3] = __dadd_rn(s4[jj & 3], ho.D[jj * kTile + lane]);
-                Eu = __dadd_rn(Eu, __dadd_rn(__dadd_rn(s4[0], s4[1]), __dadd_rn(s4[2], s4[3])));
+                for (int j = 0; j < kTile; ++j) s8[j & 7] = __dadd_rn(s8[j & 7], ((A >> j) & 1u) ? d[j] : 0.0);
+                return __dadd_rn(__dadd_rn(__dadd_rn(s8[0], s8[1]), __dadd_rn(s8[2], s8[3])),
+                                 __dadd_rn(__dadd_rn(s8[4], s8[5]), __dadd_rn(s8[6], s8[7])));
+            };
+            if (t > 0) {  // corrections of the tile just resolved: block (t, t-1)
+                Eu = __dadd_rn(Eu, masked_sum(dp, Ap));
                 ovv = ovv || (((ho.ovnP[lane] & Ap) | (ho.ovoP[lane] & ~Ap)) != 0u);
             }
             // Decisions of the 32 trials of this tile.  Trial l depends on the accept bits of the lanes j < l only
@@ -605,7 +647,6 @@ static __device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
             // each a masked sum instead of Alg. 4's 32 dependent steps.  Es < 0 is read off the
             // sign bit (Es is never -0: ln u < 0 strictly and an exact cancellation gives +0).
             const unsigned ovo = ho.ovoD[lane], ovn = ho.ovnD[lane];
-            const double* diag = ho.D + kTile * kTile;
             const double E0 = Eu;
             const bool veto0 = wallv || ovv;
             double Es = __fma_rn(lbq, E0, lnu);
@@ -613,13 +654,7 @@ static __device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
             bool hit = false;
 #pragma unroll 1
             for (int pass = 0; pass <= kTile; ++pass) {
-                double s4[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-                for (int j = 0; j < kTile; ++j) {
-                    const double dj = diag[j * kTile + lane];   // 0 for lanes <= j
-                    s4[j & 3] = __dadd_rn(s4[j & 3], ((A >> j) & 1u) ? dj : 0.0);
-                }
-                Eu = __dadd_rn(E0, __dadd_rn(__dadd_rn(s4[0], s4[1]), __dadd_rn(s4[2], s4[3])));
+                Eu = __dadd_rn(E0, masked_sum(dd, A));
                 Es = __fma_rn(lbq, Eu, lnu);
                 hit = ((ovn & A) | (ovo & ~A)) != 0u;             // bits >= lane are 0 in both words
                 const unsigned A1 = __ballot_sync(0xffffffffu, !veto0 && !hit && (__double2hiint(Es) < 0));
@@ -733,7 +768,9 @@ static __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, boo
     int* sy = a.sy;
     const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
     for (unsigned it = 1;; ++it) {
-        if ((it & 1023u) == 0u) wd_check(wd, global_ns());   // no time limit of its own: leaves when another wait gave up
+        // no time limit of its own: leaves when another wait gave up -- through an exit ITEM, not by exiting: the
+        // other threads of the CTA wait for the item at a barrier and would run the previous one again
+        if ((it & 1023u) == 0u && *(volatile int*)(sy + kSyAbort) != 0) { item[0] = kItemExit; return; }
         // one round trip: five independent loads
         const int tl = ld_relaxed(sy + kSyTicket), tu = ld_relaxed(sy + kSyTicketU), td = ld_relaxed(sy + kSyDTicket);
         const int u = ld_relaxed(sy + kSyUTicket), groups = ld_acquire(sy + kSyGroups);   // acquire: what the chain published
@@ -783,12 +820,13 @@ static __device__ __noinline__ void diag_item(const PArgs& a, PShared& sh, int c
 // counted in gbar[0]; the last one resets the count and releases the others by bumping the generation gbar[32].
 // The acquire load (LDG.STRONG.GPU + CCTL.IVALL) also drops this SM's L1, so plain loads after the barrier see
 // what the other CTAs wrote before it.
-__device__ __forceinline__ void grid_barrier(const PArgs& a) {
+__device__ __forceinline__ bool grid_barrier(const PArgs& a, PShared& sh) {
     __syncthreads();
     if (threadIdx.x == 0) {
         const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
         int* cnt = a.gbar;
         int* gen = a.gbar + 32;
+        int ok = 1;
         const int g0 = ld_acquire(gen);          // read before arriving: nobody can bump it until this CTA has arrived
         __threadfence();
         if (atomicAdd(cnt, 1) == (int)gridDim.x - 1) {
@@ -799,11 +837,13 @@ __device__ __forceinline__ void grid_barrier(const PArgs& a) {
             const unsigned long long t0 = global_ns();
             for (unsigned it = 1; ld_acquire(gen) == g0; ++it) {
                 __nanosleep(40);
-                if ((it & 1023u) == 0u) wd_check(wd, t0);
+                if ((it & 1023u) == 0u && wd_poll(wd, t0)) { ok = 0; break; }
             }
         }
+        sh.item[3] = (sh.item[3] & 1) | (ok ? 0 : 2);   // bit 1: the launch is being abandoned (a wait ran into the watchdog)
     }
     __syncthreads();
+    return (sh.item[3] & 2) == 0;      // the same in every thread of the CTA: they leave the kernel together
 }
 
 // a1 for the whole system, shared out over all threads of the grid; also clears the row accumulators
@@ -889,7 +929,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
     if (*(volatile int*)&p.st->stall) return;   // a stalled sweep invalidated the state: every later sweep is a no-op
 
     auto init_chain_barriers = [&]() {
-        for (int s = 0; s < kRing; ++s) { mbar_init(&sh.ho_bar[s], 2); mbar_init(&sh.p_bar[s], 1); }
+        for (int s = 0; s < kRing; ++s) { mbar_init(&sh.ho_bar[s], 1); mbar_init(&sh.d_bar[s], 1); mbar_init(&sh.p_bar[s], 1); }
         for (int s = 0; s < 2 * (kChunkMax / kTile); ++s) mbar_init(&sh.a_bar[0][0] + s, 1);
     };
     if (tid == 0) {
@@ -904,6 +944,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
         unsigned smid;
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
         if (blockIdx.x == 0) {
+            sh.item[3] = 0;
             st_release(a.sy + kSyChainSm, (int)smid + 1);
         } else {
             int v;
@@ -918,16 +959,16 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
     }
     __syncthreads();
     const bool is_chain = blockIdx.x == 0 && a.mode != 1;
-    const bool idle = blockIdx.x != 0 && sh.item[3] == 1 && a.mode != 1;
+    const bool idle = blockIdx.x != 0 && (sh.item[3] & 1) == 1 && a.mode != 1;
 
     unsigned kring = 0;
     for (int sw = 0; sw < a.nsweeps; ++sw) {
         trial_phase(p);
-        grid_barrier(a);
+        if (!grid_barrier(a, sh)) return;
         if (is_chain) {
             if (sw > 0) {      // the hand-off barriers start every sweep in phase 0
                 if (tid == 0) {
-                    for (int s = 0; s < 2 * kRing + 2 * (kChunkMax / kTile); ++s)
+                    for (int s = 0; s < 3 * kRing + 2 * (kChunkMax / kTile); ++s)
                         asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&sh.ho_bar[0] + s)) : "memory");
                     init_chain_barriers();
                     mbar_fence_init();
@@ -938,7 +979,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
         } else if (!idle) {
             worker_sweep<ROWS, UNIFORM, FORM>(a, sh, kring);
         }
-        grid_barrier(a);
+        if (!grid_barrier(a, sh)) return;
         // everybody is done with the scheduling words: CTA 0 clears them for the next sweep (or the next launch);
         // the election word stays until the launch ends.  The next reader is behind the next grid barrier.
         if (blockIdx.x == 0) {

@@ -134,3 +134,46 @@ def test_fp32_position_variant_matches_the_oracle_in_the_same_mode(base, N):
     ref.mc_sweep(8)
     assert not np.array_equal(ref.positions, p)
     assert hard_constraints_ok(p, d, w.cavity_R)
+
+
+@pytest.mark.parametrize("base,N", [(2, 1500), (3, 2500)])
+def test_parallel_reduction_comparison_kernel_runs_the_same_chain(base, N):
+    """the paper's comparison code -- one kernel launch per trial,
+    block reductions, atomic sub-totals, the last block decides -- gives the oracle's chain bit for bit, may be
+    mixed with mc_sweep, and costs N launches per sweep."""
+    from parity_util import assert_stats_equal
+    w = W.scaled(W.CONFIGS[base], N)
+    g, o = make_pair(w, threads=NCPU)
+
+    class ViaReduction:
+        """lockstep() drives mc_sweep; here every odd call goes through the comparison kernel instead."""
+        def __init__(self, g):
+            self.g, self.k = g, 0
+
+        def mc_sweep(self, n):
+            (self.g.mc_sweep_reduction if self.k % 2 == 0 else self.g.mc_sweep)(n)
+            self.k += 1
+
+        def __getattr__(self, name):
+            return getattr(self.g, name)
+
+        @property
+        def positions(self):
+            return self.g.positions
+
+        @property
+        def sweep_index(self):
+            return self.g.sweep_index
+
+        @sweep_index.setter
+        def sweep_index(self, s):
+            self.g.sweep_index = s
+
+    from parity_util import lockstep
+    l0 = g.mc_get_launch_count()
+    r = lockstep(ViaReduction(g), o, 6, tag="parallel reduction")
+    record_margin(f"parallel_reduction_{w.name}", N=w.N, sweeps=6, max_dE_err=r["max_dE_err"])
+    assert_stats_equal(g, o, r["near_tie_flips"])
+    assert g.sweep_index == 6
+    assert g.mc_get_launch_count() - l0 >= 3 * w.N          # three of the six sweeps took N launches each
+    assert abs(g.mc_get_stats()["E_running"] - g.mc_energy()) <= 1e-9 * abs(g.mc_energy())
