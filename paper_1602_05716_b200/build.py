@@ -40,6 +40,7 @@ def build_extension(force: bool = False, verbose: bool = False) -> Path:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     OBJDIR.mkdir(exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
+    extra += os.environ.get("MCB_NVCC_FLAGS", "").split()     # e.g. -DMCB_COLS_PER_ITER=2 for an experiment
 
     def compile_unit(unit):
         name, src, defs = unit

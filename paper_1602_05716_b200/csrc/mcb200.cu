@@ -51,9 +51,9 @@ Layout make_layout(int64_t N) {
     const size_t nt = kChunkMax / kTile;
     L.xy = take(Np * 16); L.zq = take(Np * 16); L.hh = take(Np * 8); L.lbq = take(Np * 8);
     L.txy = take(Np * 16); L.tz = take(Np * 8); L.lnu = take(Np * 8); L.wall = take(Np);
-    // double-buffered by chunk parity (the sweep kernel prepares chunk c+1 while the chain is in c)
-    L.Dblk = take(2 * (nt * (nt + 1) / 2) * kTile * kTile * 8);
-    L.OVold = take((size_t)2 * kChunkMax * nt * 4); L.OVnew = take((size_t)2 * kChunkMax * nt * 4);
+    // a ring of kDRing buffers by chunk index (the sweep kernel prepares the next chunks while the chain is in c)
+    L.Dblk = take((size_t)kDRing * (nt * (nt + 1) / 2) * kTile * kTile * 8);
+    L.OVold = take((size_t)kDRing * kChunkMax * nt * 4); L.OVnew = take((size_t)kDRing * kChunkMax * nt * 4);
     L.S1 = take(Np * 8); L.S2 = take(Np * 8); L.ovc = take(Np * 4); L.nn = take(Np * 8);
     L.sy = take((size_t)2 * (kSyHdr + 4 * (Np / 256 + 1)) * 4);   // live words + snapshot of the last completed sweep
     L.gbar = take(256);

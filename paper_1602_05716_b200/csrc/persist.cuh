@@ -27,6 +27,10 @@ constexpr int kFixCols = 16;                   // columns per FIX item (columns 
 constexpr int kMidCols = 32;                   // columns per MID item (columns of chunk c-2)
 constexpr int kRing = 4;                       // hand-off ring depth of the chain CTA
 constexpr int kHelpers = 6;
+#ifndef MCB_DRING
+#define MCB_DRING 4
+#endif
+constexpr int kDRing = MCB_DRING;                      // D / overlap-bit buffers: DIAG(c) may run once the chain has finished chunk c - kDRing
 #ifndef MCB_COLS_PER_ITER
 #define MCB_COLS_PER_ITER 4
 #endif
@@ -167,7 +171,8 @@ struct __align__(128) PShared {
     uint64_t p_bar[kRing];                // publisher done with the slot
     uint64_t a_bar[2][kChunkMax / kTile]; // accept mask of tile t of a chunk (by chunk parity) published
     unsigned sA[2][kChunkMax / kTile];
-    int item[4];
+    int pub_gt;       // chain CTA: 1 + the last tile the publisher has taken out of its slot (monotonic within a sweep)
+    int item[4];      // [0] type, [1] chunk, [2] index, [3] CTA flags (bit 0 idle, bit 1 abandoned)
 };
 
 __device__ __forceinline__ int* sy_far_done(const PArgs& a) { return a.sy + kSyHdr; }
@@ -180,7 +185,7 @@ struct ChunkBufs {
     unsigned* OVold; unsigned* OVnew;   // [C][C / 32]
 };
 __device__ __forceinline__ ChunkBufs chunk_bufs(const PArgs& a, int c) {
-    const size_t b = (size_t)(c & 1);
+    const size_t b = (size_t)(c % kDRing);
     const size_t nt = kChunkMax / kTile;
     ChunkBufs B;
     B.Dblk = a.p.Dblk + b * (nt * (nt + 1) / 2) * (kTile * kTile);
@@ -409,7 +414,7 @@ namespace mcb {
 // helper warp of the chain CTA: prepares row tile t of chunk c and hands it over
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, const ChunkBufs& B, int c, int t,
-                                                  int row0, int gt) {
+                                                  int row0, int gt, bool first) {
     const int lane = threadIdx.x & 31;
     const int C = a.C, W = C / kTile;
     const int r = t * kTile + lane, i = row0 + r;
@@ -418,9 +423,8 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
     const unsigned apar = (unsigned)(c >> 1) & 1u;
     const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
 
-    // base sum of all FAR, FIX and DIAG items of this row
-    double E = accum_value(__ldcg(a.p.S1 + i), __ldcg(a.p.S2 + i));
-    unsigned veto = (unsigned)a.p.wall[i] | (__ldcg(a.p.ovc + i) > 0 ? kFlagOverlap : 0u);
+    // what depends on the trial phase and the chunk's DIAG items only
+    unsigned veto = (unsigned)a.p.wall[i];
     const double lbq = a.p.lbq[i], lnu = a.p.lnu[i];
     const double2 txy = a.p.txy[i];
     const double tz = a.p.tz[i];
@@ -430,8 +434,19 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
 
     bool staged = false;
     auto stage_blocks = [&]() {
-        // the slot is free once the publisher is done with tile gt - kRing
-        if (gt >= kRing) mbar_wait_wd(wd, &sh.p_bar[slot], (unsigned)(gt / kRing - 1) & 1u);
+        // the slot is free once the publisher is done with tile gt - kRing.  A parity wait alone would be fooled if
+        // this warp were two tiles of the slot ahead of the publisher (it can be, at the start of a chunk), so the
+        // monotonic tile counter is checked first; the mbarrier then only orders the publisher's reads before the copy
+        if (gt >= kRing) {
+            if (*(volatile int*)&sh.pub_gt < gt - kRing + 1) {
+                const unsigned long long t0 = global_ns();
+                for (unsigned it = 1; *(volatile int*)&sh.pub_gt < gt - kRing + 1; ++it) {
+                    __nanosleep(32);
+                    if ((it & 1023u) == 0u) wd_check(wd, t0);
+                }
+            }
+            mbar_wait_wd(wd, &sh.p_bar[slot], (unsigned)(gt / kRing - 1) & 1u);
+        }
         if (lane == 0) {
             const int nb = min(t, 2) + 1;          // blocks (t, t-2), (t, t-1), (t, t): contiguous in Dblk
             const double* src = B.Dblk + (size_t)blk_index(t, t + 1 - nb) * (kTile * kTile);
@@ -442,6 +457,26 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
         }
         staged = true;
     };
+
+#ifndef MCB_PRESTAGE
+#define MCB_PRESTAGE 1
+#endif
+    if (first) {
+        // this helper's first tile of the chunk: the block copy is under way while the chunk's last FAR and
+        // urgent items complete (every lane polls -- one broadcast load: the warp waits, and gives up, as a whole)
+        if (MCB_PRESTAGE) stage_blocks();
+        const long long t0 = clock64();
+        spin_until_ge(wd, sy_far_done(a) + c, far_items(a.p.Np, C, a.farcols, a.nfar, c));
+        const long long t1 = clock64();
+        if (c > 0) spin_until_ge(wd, sy_fix_done(a) + c, urgent_items(C, c));
+        if (t == 0 && lane == 0 && a.dbg) {
+            a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t1;
+            if (c < 300) a.dbg[16 + 3 * c] = (long long)global_ns();   // inputs of chunk c complete
+        }
+    }
+    // base sum of all FAR, FIX and DIAG items of this row
+    double E = accum_value(__ldcg(a.p.S1 + i), __ldcg(a.p.S2 + i));
+    if (__ldcg(a.p.ovc + i) > 0) veto |= kFlagOverlap;
 
     // corrections of the column tiles s <= t - 3, as their accept masks appear (masked loads from L2)
     for (int s = 0; s + 3 <= t; ++s) {
@@ -510,7 +545,10 @@ __device__ __forceinline__ void chain_publisher(const PArgs& a, PShared& sh) {
             const double2 t2 = ho.txy[lane];
             const double tz = ho.tz[lane];
             __syncwarp();
-            if (lane == 0) mbar_arrive(&sh.p_bar[slot]);      // the slot is free for tile gt + kRing before the global stores below
+            if (lane == 0) {      // the slot is free for tile gt + kRing before the global stores below
+                mbar_arrive(&sh.p_bar[slot]);
+                *(volatile int*)&sh.pub_gt = gt + 1;
+            }
             if (fl & kFlagAccept) {
                 p.xy[i] = t2;
                 p.zq[i].x = tz;
@@ -581,21 +619,13 @@ static __device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
         for (int c = 0; c < a.nchunks; ++c) {
             const int row0 = c * C, nrows = chunk_rows(p.Np, C, c), nt = nrows / kTile;
             if (h >= nt) continue;
-            {   // every lane polls (one broadcast load): the warp waits, and gives up, as a whole
+            {
                 const long long t0 = clock64();
-                spin_until_ge(wd, sy_far_done(a) + c, far_items(p.Np, C, a.farcols, a.nfar, c));
-                const long long t1 = clock64();
                 spin_until_ge(wd, sy_diag_done(a) + c, diag_items(nrows));
-                const long long t2 = clock64();
-                if (c > 0) spin_until_ge(wd, sy_fix_done(a) + c, urgent_items(C, c));
-                if (h == 0 && lane == 0 && a.dbg) {
-                    a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t2; a.dbg[15] += t2 - t1;
-                    if (c < 300) a.dbg[16 + 3 * c] = (long long)global_ns();   // inputs of chunk c complete
-                }
+                if (h == 0 && lane == 0 && a.dbg) a.dbg[15] += clock64() - t0;
             }
-            __syncwarp();
             const ChunkBufs B = chunk_bufs(a, c);
-            for (int t = h; t < nt; t += kHelpers) chain_helper_tile(a, sh, B, c, t, row0, c * ntfull + t);
+            for (int t = h; t < nt; t += kHelpers) chain_helper_tile(a, sh, B, c, t, row0, c * ntfull + t, t == h);
         }
         return;
     }
@@ -689,12 +719,12 @@ namespace mcb {
 enum { kItemExit = 0, kItemDiag = 1, kItemFarL = 2, kItemFix = 3, kItemFarU = 4, kItemMid = 5 };
 
 // Work queues.  Each is a ticket counter in global memory; tickets run through the chunks in order.
-//   QL  FAR items over the columns before chunk c-1 (final positions): released when the chain
-//       has finished chunk c-2
-//   QU  FAR items over the columns after chunk c (sweep-start positions): never blocked -- the
+//   QL  FAR-L items over the columns before chunk c-2 (final positions): released when the chain
+//       has finished chunk c-3
+//   QU  FAR-U items over the columns after chunk c (sweep-start positions): never blocked -- the
 //       filler that keeps every SM busy while the chain works
-//   QD  DIAG items: released with QL (the D buffers are double-buffered by chunk parity)
-//   FIX urgent items: exist as soon as the chain has published their 16 columns
+//   QD  DIAG items: released when the chain has finished chunk c - kDRing (ring of D buffers)
+//   FIX / MID urgent items: exist as soon as the chain has published their columns
 // Thread 0 of a worker CTA reads all five words (four counters and the chain's progress) in one
 // round trip, picks the first queue whose next ticket is released -- FIX/MID, QD, QL, QU for the
 // FAR workers (what the chain needs soonest first); FIX/MID, QD for the a.nnear "near" workers that
@@ -723,10 +753,10 @@ __device__ __forceinline__ void advance(const PArgs& a, Cursor& cur, int t) {
         ++cur.c;
     }
 }
-// QL items of chunk c need the chain to have finished chunk c-3, QD items chunk c-2 (buffer parity)
+// QL items of chunk c need the chain to have finished chunk c-3, QD items chunk c - kDRing (buffer ring)
 template <int Q>
 __device__ __forceinline__ bool released(const PArgs& a, int c, int groups) {
-    return Q == QL ? (c < 3 || groups >= (c - 2) * (a.C / kGroup)) : (c < 2 || groups >= (c - 1) * (a.C / kGroup));
+    return Q == QL ? (c < 3 || groups >= (c - 2) * (a.C / kGroup)) : (c < kDRing || groups >= (c - kDRing + 1) * (a.C / kGroup));
 }
 
 // t = the counter's value as just read, groups = the chain's progress as just read.
@@ -766,7 +796,6 @@ static __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, boo
     const int C = a.C, GPC = C / kGroup, nfix = C / kFixCols, nmid = C / kMidCols;
     const int total_urgent = a.nchunks >= 2 ? nfix + (a.nchunks - 2) * (nfix + nmid) : 0;
     int* sy = a.sy;
-    const Watch wd{a.sy, a.p.st, a.p.wait_limit_ns};
     for (unsigned it = 1;; ++it) {
         // no time limit of its own: leaves when another wait gave up -- through an exit ITEM, not by exiting: the
         // other threads of the CTA wait for the item at a barrier and would run the previous one again
@@ -931,6 +960,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
     auto init_chain_barriers = [&]() {
         for (int s = 0; s < kRing; ++s) { mbar_init(&sh.ho_bar[s], 1); mbar_init(&sh.d_bar[s], 1); mbar_init(&sh.p_bar[s], 1); }
         for (int s = 0; s < 2 * (kChunkMax / kTile); ++s) mbar_init(&sh.a_bar[0][0] + s, 1);
+        *(volatile int*)&sh.pub_gt = 0;
     };
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) {
