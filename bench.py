@@ -329,6 +329,12 @@ def run_ours(args, w):
     # mc_sweep(n) is ONE launch: the per-sweep cost without the launch (what paces the small configurations)
     n_multi = max(2, min(100, w.sweeps))
     multi_ms = min(sysm.mc_sweep_timed(n_multi) for _ in range(3)) / n_multi
+    # the paper's comparison code (one kernel launch per trial, parallel reduction), one sweep
+    ev0.record(stream)
+    sysm.mc_sweep_reduction(1)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    red_ms = ev0.elapsed_time(ev1)
     form = sysm.mc_get_option("form")
     executed = EXECUTED_FP64_PER_PAIR[form][0 if sysm.mc_get_option("uniform_path") else 1]
     prop = torch.cuda.get_device_properties(dev)
@@ -383,6 +389,9 @@ def run_ours(args, w):
         "multi_sweep_launch": {"sweeps_per_launch": n_multi, "ms_per_sweep": multi_ms,
                                "value": pairs_per_step / (multi_ms * 1e-3), "unit": UNIT,
                                "fp64_roofline_frac": pairs_per_step / (multi_ms * 1e-3) * FP64_INSTR_PER_PAIR / peak_instr},
+        "comparison_parallel_reduction": {"ms_per_sweep": red_ms, "launches_per_sweep": N,
+                                          "value": pairs_per_step / (red_ms * 1e-3), "unit": UNIT,
+                                          "note": "the paper's comparison code (PAPER.md:278-282), same chain; context, not the product path"},
         "clocks": {k: clocks[k] for k in ("sm_mhz", "sm_max_mhz", "reasons")},
         "e2e": {"value": units_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps},

@@ -169,8 +169,8 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
  * the partition of a row's sum change dE by rounding only (the sums themselves do not depend on the
  * schedule).  Unknown keys and out-of-range values return MC_EINVAL.
  *   "prows"        1|2|4   rows per thread of the sweep kernel; chunk = 256 * prows rows
- *                          (default by N: 4 from 16384, 2 from 2048, else 1)
- *   "far_cols"     8..65536, multiple of 8: target columns per FAR item (default 256)
+ *                          (default by N: 4 from 32768, 2 from 512, else 1)
+ *   "far_cols"     8..65536, multiple of 8: target columns per FAR item (default 256 from N = 32768, else 64)
  *   "pnear"        0..128  worker CTAs that serve only urgent and in-chunk items (default 4)
  *   "wave"         0|1     round a chunk's FAR items to a multiple of the FAR workers (default 1)
  *   "form"         -1|0|1|2  pair-distance form (persist.cuh): -1 = by geometry (default): 0 GRAM if
@@ -184,6 +184,9 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
  *   "uniform_path" 0|1     allow the equal-diameter specialisation (default 1)
  *   "stall_ms"     0..3600000  watchdog limit per wait of the sweep kernel in ms (default 2000; 0 = none;
  *                          raise it under a profiler, a sanitizer or GPU time-slicing)
+ *   "diag_split"   0|1|2|4|8  warps that share one 32 x 32 in-chunk unit of the sweep kernel, each taking a part of
+ *                          its columns -- the multi-thread-per-particle scheme of PAPER.md:243-245 for systems too
+ *                          small to fill the device (0 = by N: 8 up to 2048 ions, 4 up to 8192, 2 up to 32768, else 1)
  *   "max_ctas"     0..4096 upper limit on the CTAs of the sweep kernel (0 = two per SM, the default for large
  *                          systems; small systems synchronise faster on a smaller grid)
  *   "energy_rows"  4|6|8   rows per thread of the from-scratch energy kernel

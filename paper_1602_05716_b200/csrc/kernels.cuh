@@ -125,10 +125,15 @@ __device__ __forceinline__ int blk_index(int t, int s) { return t * (t + 1) / 2 
 
 // one (row tile t, column tile s) unit, executed by one warp; the five arrays are this warp's
 // 32-entry shared-memory staging rows
+// Columns jj0 <= jj < jj1 of the unit only: several warps may share a unit (the multi-thread-per-particle idea of
+// the terms of one trial spread over eta "slave" threads when the system is too small to
+// fill the device); ovo / ovn return this part's overlap bits, which the caller combines over the parts.
 __device__ __forceinline__ void diag_unit(const Params& p, int row0, int nrows, int unit, double2* cxy, double2* czq,
-                                          double2* ctxy, double* ch, double* ctz) {
+                                          double2* ctxy, double* ch, double* ctz, int jj0, int jj1, unsigned& ovo_out,
+                                          unsigned& ovn_out) {
     const int lane = threadIdx.x & 31;
     const int nt = nrows / kTile;
+    ovo_out = 0u; ovn_out = 0u;
     if (unit >= nt * nt) return;
     const int t = unit / nt, s = unit % nt;
     const int r = t * kTile + lane, i = row0 + r;
@@ -145,13 +150,12 @@ __device__ __forceinline__ void diag_unit(const Params& p, int row0, int nrows, 
     const double xi = xyi.x, yi = xyi.y, zi = p.zq[i].x;
     const double txi = txyi.x, tyi = txyi.y, tzi = p.tz[i];
     const double hi = p.hh[i];
-    const int W = p.chunk / kTile;
     double bsum = 0.0;
     int ovc = 0;
     unsigned ovo = 0u, ovn = 0u;
     double* blk = (s <= t) ? p.Dblk + (size_t)blk_index(t, s) * (kTile * kTile) : nullptr;
 #pragma unroll 4
-    for (int jj = 0; jj < kTile; ++jj) {
+    for (int jj = jj0; jj < jj1; ++jj) {
         const double2 a = cxy[jj];
         const double2 b = czq[jj];
         const double sij = __dadd_rn(hi, ch[jj]);
@@ -183,10 +187,7 @@ __device__ __forceinline__ void diag_unit(const Params& p, int row0, int nrows, 
         if (s == t && jj > lane) blk[jj * kTile + lane] = 0.0;
     }
     accum_row(p, i, bsum, ovc);
-    if (s <= t) {
-        p.OVold[(size_t)r * W + s] = ovo;
-        p.OVnew[(size_t)r * W + s] = ovn;
-    }
+    ovo_out = ovo; ovn_out = ovn;
 }
 
 

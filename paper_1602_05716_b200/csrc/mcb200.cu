@@ -80,6 +80,7 @@ struct mc_handle {
     int num_sms = 148;
     int prows = 4;           // rows per consumer thread of the sweep kernel (chunk = 256 * prows)
     int pfarcols = 256;      // columns per FAR item of the sweep kernel
+    int dsplit = 0;          // warps per DIAG unit of the sweep kernel (0: by N)
     int erows = 4;           // rows per thread of k_energy (Gram form)
     int hist_slices = kHistSlices;   // column slices (grid.y) of k_hist
     int pmode = 0;           // 1: throughput probe (diagnostic, needs "debug"; the sweep's results are meaningless)
@@ -135,6 +136,7 @@ int launch_sweep(mc_handle* h, cudaStream_t s, int nsweeps) {
     a.farcols = h->pfarcols;
     a.mode = h->pmode;
     a.nfar = h->pwave ? std::max(1, h->pgrid - 2 - a.nnear) : 0;
+    a.dsplit = h->dsplit > 0 ? h->dsplit : (a.p.Np <= 2048 ? 8 : a.p.Np <= 8192 ? 4 : a.p.Np <= 32768 ? 2 : 1);
     a.nsweeps = nsweeps;
     a.sy = h->p.sy;
     a.gbar = (int*)(h->ws + h->L.gbar);
@@ -238,7 +240,10 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     p.nn = (double*)(w + L.nn);
     p.S1 = (long long*)(w + L.S1); p.S2 = (long long*)(w + L.S2); p.ovc = (int*)(w + L.ovc);
     p.sy_n = kSyHdr + 4 * (p.Np / 256 + 1);   // header + per-chunk counters
-    h->prows = p.Np >= 16384 ? 4 : (p.Np >= 2048 ? 2 : 1);
+    // measured on B200: 1024-row chunks and 256-column items pay only when the pair work fills the
+    // device; below that the chain paces the sweep and shorter chunks and items keep its inputs ahead of it
+    h->prows = p.Np >= 32768 ? 4 : (p.Np >= 512 ? 2 : 1);
+    h->pfarcols = p.Np >= 32768 ? 256 : 64;
     p.R = cavity_R; p.lB = bjerrum_length; p.max_disp = max_disp; p.seed = seed;
     p.wait_limit_ns = 2000000000ull;
     p.pos_bits = 64;
@@ -533,6 +538,9 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     } else if (!std::strcmp(key, "pnear")) {
         if (value < 0 || value > 128) return fail(MC_EINVAL, "pnear must be in 0..128");
         h->pnear = (int)value;
+    } else if (!std::strcmp(key, "diag_split")) {
+        if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) return fail(MC_EINVAL, "diag_split must be 0 (by N), 1, 2, 4 or 8");
+        h->dsplit = (int)value;
     } else if (!std::strcmp(key, "max_ctas")) {
         if (value < 0 || value > 4096) return fail(MC_EINVAL, "max_ctas must be in 0..4096 (0: two per SM)");
         h->max_ctas = (int)value;
@@ -586,6 +594,7 @@ int mc_get_option(mc_handle* h, const char* key, int64_t* value_host) {
     else if (!std::strcmp(key, "pnear")) *value_host = h->pnear;
     else if (!std::strcmp(key, "wave")) *value_host = h->pwave ? 1 : 0;
     else if (!std::strcmp(key, "max_ctas")) *value_host = h->max_ctas;
+    else if (!std::strcmp(key, "diag_split")) *value_host = h->dsplit;
     else if (!std::strcmp(key, "form")) *value_host = h->form;
     else if (!std::strcmp(key, "form_auto")) *value_host = h->form_auto;
     else if (!std::strcmp(key, "position_bits")) *value_host = h->p.pos_bits;
@@ -641,7 +650,7 @@ int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers,
         if (urgent_items(C, c) != (c >= 2 ? C / kMidCols : 0) + (c >= 1 ? C / kFixCols : 0)) ++violations;
         // DIAG covers the chunk's own columns
         for (int k = row0 / 8; k < (row0 + nrows) / 8; ++k) ++cover[k];
-        items += diag_items(nrows);
+        items += diag_items(nrows, 1);
         for (int k = 0; k < Np / 8; ++k) violations += cover[k] != 1;
     }
     out4_host[0] = items; out4_host[1] = violations; out4_host[2] = max_item_cols; out4_host[3] = urgent;

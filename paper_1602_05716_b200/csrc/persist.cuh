@@ -50,6 +50,7 @@ struct PArgs {
     int nfar;         // number of FAR workers (0: do not round item counts to it)
     int mode;         // 0 normal; 1 throughput probe: no chain, every CTA runs QU items over all columns but the chunk's own;
                       // 2 watchdog test: the deciding warp never runs, so the sweep stalls
+    int dsplit;       // warps that share one DIAG unit: 1, 2, 4 or 8
     int nsweeps;      // sweeps this launch runs (a1-a4 each), separated by grid-wide barriers
     int* sy;          // [kSyHdr + 3 * nchunks]: header, far_done, diag_done, fix_done; all zero at launch and again at exit
     int* gbar;        // grid barrier: [0] arrivals, [32] generation
@@ -78,9 +79,10 @@ __host__ __device__ inline int probe_cols(int Np, int C, int c) { return Np - ch
 __host__ __device__ inline int far_items(int Np, int C, int farcols, int nfar, int c) {
     return far_slices(farL_cols(C, c), farcols, nfar) + far_slices(farU_cols(Np, C, c), farcols, nfar);
 }
-__host__ __device__ inline int diag_items(int nrows) {
+// DIAG items of a chunk: nt x nt units of 32 x 32, each shared by `split` warps (1, 2, 4 or 8), 8 warps per item
+__host__ __device__ inline int diag_items(int nrows, int split) {
     const int nt = nrows / kTile;
-    return (nt * nt + 7) / 8;
+    return (nt * nt * split + 7) / 8;
 }
 
 __device__ __forceinline__ int ld_acquire(const int* p) {
@@ -162,6 +164,7 @@ struct __align__(128) PShared {
             ColStage stage[kStages];
             double2 cxy[8][32], czq[8][32], ctxy[8][32];
             double ch[8][32], ctz[8][32];
+            unsigned ov[8][2][32];
         } w;
         HandOff ho[kRing];
     } u;
@@ -621,7 +624,7 @@ static __device__ __noinline__ void chain_cta(const PArgs& a, PShared& sh) {
             if (h >= nt) continue;
             {
                 const long long t0 = clock64();
-                spin_until_ge(wd, sy_diag_done(a) + c, diag_items(nrows));
+                spin_until_ge(wd, sy_diag_done(a) + c, diag_items(nrows, a.dsplit));
                 if (h == 0 && lane == 0 && a.dbg) a.dbg[15] += clock64() - t0;
             }
             const ChunkBufs B = chunk_bufs(a, c);
@@ -744,7 +747,7 @@ template <int Q>
 __device__ __forceinline__ int items_of(const PArgs& a, int c) {
     return Q == QL ? far_slices(farL_cols(a.C, c), a.farcols, a.nfar)
          : Q == QU ? far_slices(a.mode == 1 ? probe_cols(a.p.Np, a.C, c) : farU_cols(a.p.Np, a.C, c), a.farcols, a.nfar)
-                   : diag_items(chunk_rows(a.p.Np, a.C, c));
+                   : diag_items(chunk_rows(a.p.Np, a.C, c), a.dsplit);
 }
 template <int Q>
 __device__ __forceinline__ void advance(const PArgs& a, Cursor& cur, int t) {
@@ -834,15 +837,33 @@ static __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, boo
     }
 }
 
-// DIAG item k of chunk c: 8 units (row tile, column tile), one per warp
+// DIAG item k of chunk c: 8 / dsplit units (row tile, column tile), each shared by dsplit warps that take
+// 32 / dsplit of its columns each (small systems: more, shorter items -- the eta scheme of PAPER.md:243-245)
 static __device__ __noinline__ void diag_item(const PArgs& a, PShared& sh, int c, int k, int row0, int nrows) {
-    const int warp = threadIdx.x >> 5;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const ChunkBufs B = chunk_bufs(a, c);
     Params pc = a.p;
     pc.chunk = a.C;
     pc.Dblk = B.Dblk; pc.OVold = B.OVold; pc.OVnew = B.OVnew;
-    diag_unit(pc, row0, nrows, k * 8 + warp, sh.u.w.cxy[warp], sh.u.w.czq[warp], sh.u.w.ctxy[warp],
-                    sh.u.w.ch[warp], sh.u.w.ctz[warp]);
+    const int split = a.dsplit, part = warp % split, per = kTile / split;
+    const int unit = (k * 8 + warp) / split;
+    unsigned ovo, ovn;
+    diag_unit(pc, row0, nrows, unit, sh.u.w.cxy[warp], sh.u.w.czq[warp], sh.u.w.ctxy[warp], sh.u.w.ch[warp],
+              sh.u.w.ctz[warp], part * per, (part + 1) * per, ovo, ovn);
+    // the parts' overlap bits, combined by the first warp of the unit
+    sh.u.w.ov[warp][0][lane] = ovo;
+    sh.u.w.ov[warp][1][lane] = ovn;
+    __syncthreads();
+    const int nt = nrows / kTile;
+    if (part == 0 && unit < nt * nt) {
+        for (int q = 1; q < split; ++q) { ovo |= sh.u.w.ov[warp + q][0][lane]; ovn |= sh.u.w.ov[warp + q][1][lane]; }
+        const int t = unit / nt, s2 = unit % nt;
+        if (s2 <= t) {
+            const int W = a.C / kTile, r = t * kTile + lane;
+            B.OVold[(size_t)r * W + s2] = ovo;
+            B.OVnew[(size_t)r * W + s2] = ovn;
+        }
+    }
 }
 
 // Grid-wide barrier between the phases of a launch (all CTAs are co-resident: cooperative launch).  Arrivals are
@@ -1019,7 +1040,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
                 int bad = 0;
                 for (int c = tid; c < a.nchunks; c += kPThreads) {
                     bad |= a.sy[kSyHdr + c] != far_items(p.Np, a.C, a.farcols, a.nfar, c);
-                    bad |= a.sy[kSyHdr + a.nchunks + c] != diag_items(chunk_rows(p.Np, a.C, c));
+                    bad |= a.sy[kSyHdr + a.nchunks + c] != diag_items(chunk_rows(p.Np, a.C, c), a.dsplit);
                     bad |= a.sy[kSyHdr + 2 * a.nchunks + c] != urgent_items(a.C, c);
                 }
                 if (__syncthreads_or(bad) && tid == 0) p.st->sched_mismatch += 1;

@@ -367,7 +367,8 @@ def test_strong_coupling_low_acceptance():
     # rows per thread / chunk size, item width, near workers, wave rounding, pair-distance form, diameter path
     {"prows": 1}, {"prows": 2}, {"prows": 4}, {"far_cols": 64}, {"far_cols": 1024}, {"pnear": 0}, {"pnear": 32},
     {"wave": 0}, {"prows": 2, "far_cols": 8, "pnear": 1}, {"debug": 1}, {"form": 1}, {"form": 2},
-    {"form": 1, "prows": 1}, {"form": 2, "prows": 4}, {"uniform_path": 0, "form": 2}])
+    {"form": 1, "prows": 1}, {"form": 2, "prows": 4}, {"uniform_path": 0, "form": 2},
+    {"diag_split": 1}, {"diag_split": 2}, {"diag_split": 8, "prows": 1}, {"max_ctas": 32}, {"max_ctas": 9, "diag_split": 4}])
 @pytest.mark.parametrize("base", [2, 3])      # two diameters / equal diameters (the specialised path)
 def test_every_launch_configuration_gives_the_same_chain(opts, base):
     w = W.scaled(W.CONFIGS[base], 2500)
@@ -389,6 +390,7 @@ def test_persistent_kernel_is_bit_reproducible(N, prows):
     for rep in range(3):
         g = MCSystem(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 5)
         g.mc_set_option("prows", prows)
+        g.mc_set_option("wave", 0)                    # item counts independent of the number of FAR workers
         g.mc_set_option("pnear", (0, 4, 16)[rep])     # perturbs the schedule, not the items
         g.mc_sweep(6)
         lg = g.mc_get_trial_log()
@@ -429,7 +431,8 @@ def test_soak_completion_counters_after_every_sweep(N, pnear):
             # the plan: diag items = ceil(nt^2 / 8); urgent = C/32 (c >= 2) + C/16 (c >= 1); far from the first sweep,
             # cross-checked against the total mc_plan_check reports
             nt = [min(C_, Np - c * C_) // 32 for c in range(nchunks)]
-            want_diag = np.array([(t * t + 7) // 8 for t in nt])
+            split = {True: 8, False: 4 if Np <= 8192 else 2 if Np <= 32768 else 1}[Np <= 2048]   # warps per DIAG unit, by N
+            want_diag = np.array([(t * t * split + 7) // 8 for t in nt])
             want_fix = np.array([(C_ // 32 if c >= 2 else 0) + (C_ // 16 if c >= 1 else 0) for c in range(nchunks)])
             assert np.array_equal(diag, want_diag) and np.array_equal(fix, want_fix)
             want = (far.copy(), want_diag, want_fix)
@@ -454,6 +457,7 @@ def test_far_item_count_matches_the_host_plan():
         w = W.scaled(W.CONFIGS[3], N)
         pos, q, d = w.arrays()
         g = MCSystem(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 1)
+        g.mc_set_option("diag_split", 1)                 # the host plan counts one warp per in-chunk unit
         g.mc_sweep(1)
         g.synchronize()
         rows = g.mc_get_option("prows")
