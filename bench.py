@@ -330,11 +330,13 @@ def run_ours(args, w):
     n_multi = max(2, min(100, w.sweeps))
     multi_ms = min(sysm.mc_sweep_timed(n_multi) for _ in range(3)) / n_multi
     # the paper's comparison code (one kernel launch per trial, parallel reduction), one sweep
-    ev0.record(stream)
-    sysm.mc_sweep_reduction(1)
-    ev1.record(stream)
-    torch.cuda.synchronize()
-    red_ms = ev0.elapsed_time(ev1)
+    red_ms = None
+    if not args.skip_comparison:
+        ev0.record(stream)
+        sysm.mc_sweep_reduction(1)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        red_ms = ev0.elapsed_time(ev1)
     form = sysm.mc_get_option("form")
     executed = EXECUTED_FP64_PER_PAIR[form][0 if sysm.mc_get_option("uniform_path") else 1]
     prop = torch.cuda.get_device_properties(dev)
@@ -389,9 +391,9 @@ def run_ours(args, w):
         "multi_sweep_launch": {"sweeps_per_launch": n_multi, "ms_per_sweep": multi_ms,
                                "value": pairs_per_step / (multi_ms * 1e-3), "unit": UNIT,
                                "fp64_roofline_frac": pairs_per_step / (multi_ms * 1e-3) * FP64_INSTR_PER_PAIR / peak_instr},
-        "comparison_parallel_reduction": {"ms_per_sweep": red_ms, "launches_per_sweep": N,
-                                          "value": pairs_per_step / (red_ms * 1e-3), "unit": UNIT,
-                                          "note": "the paper's comparison code (PAPER.md:278-282), same chain; context, not the product path"},
+        "comparison_parallel_reduction": None if red_ms is None else {
+            "ms_per_sweep": red_ms, "launches_per_sweep": N, "value": pairs_per_step / (red_ms * 1e-3), "unit": UNIT,
+            "note": "the paper's comparison code (PAPER.md:278-282), same chain; context, not the product path"},
         "clocks": {k: clocks[k] for k in ("sm_mhz", "sm_max_mhz", "reasons")},
         "e2e": {"value": units_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps},
@@ -428,6 +430,8 @@ def main(argv=None):
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--skip-cpu-baseline", action="store_true",
                     help="leave out the oracle timing (profiling runs under ncu only)")
+    ap.add_argument("--skip-comparison", action="store_true",
+                    help="leave out the sweep through the paper's one-launch-per-trial comparison kernel (N launches)")
     args = ap.parse_args(argv)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
         return spawn_replicas(args.gpus, list(sys.argv[1:] if argv is None else argv))

@@ -82,7 +82,7 @@ struct mc_handle {
     int pfarcols = 256;      // columns per FAR item of the sweep kernel
     int dsplit = 0;          // warps per DIAG unit of the sweep kernel (0: by N)
     int erows = 4;           // rows per thread of k_energy (Gram form)
-    int hist_slices = kHistSlices;   // column slices (grid.y) of k_hist
+    int hist_slices = 64;   // column slices (grid.y) of k_hist
     int pmode = 0;           // 1: throughput probe (diagnostic, needs "debug"; the sweep's results are meaningless)
     bool pwave = true;       // round the FAR items of a chunk to a multiple of the FAR workers
     int pnear = 4;           // worker CTAs of the sweep kernel that serve urgent and DIAG items only
@@ -530,7 +530,7 @@ int mc_measure_fp64_peak(void* stream, double millis, double* dfma_per_second_ho
 int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     if (!h || !key) return fail(MC_EINVAL, "null argument");
     if (!std::strcmp(key, "prows")) {
-        if (value != 1 && value != 2 && value != 4) return fail(MC_EINVAL, "prows must be 1, 2 or 4");
+        if (value < 1 || value > 4) return fail(MC_EINVAL, "prows must be 1, 2, 3 or 4");
         h->prows = (int)value;
     } else if (!std::strcmp(key, "far_cols")) {
         if (value < 8 || value > 65536 || value % 8) return fail(MC_EINVAL, "far_cols must be a multiple of 8 in 8..65536");
@@ -618,7 +618,7 @@ int mc_debug_counters(mc_handle* h, int64_t* out16_host) {
 
 int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers, int64_t* out4_host) {
     if (N < 1 || N > (int64_t)1 << 30 || !out4_host) return fail(MC_EINVAL, "bad argument");
-    if (rows_per_thread != 1 && rows_per_thread != 2 && rows_per_thread != 4) return fail(MC_EINVAL, "rows_per_thread must be 1, 2 or 4");
+    if (rows_per_thread < 1 || rows_per_thread > 4) return fail(MC_EINVAL, "rows_per_thread must be 1, 2, 3 or 4");
     if (far_cols < 8 || far_cols % 8 || far_workers < 0) return fail(MC_EINVAL, "far_cols must be a positive multiple of 8, far_workers >= 0");
     const int Np = padded(N), C = 256 * rows_per_thread, nchunks = (Np + C - 1) / C;
     int64_t items = 0, violations = 0, max_item_cols = 0, urgent = 0;

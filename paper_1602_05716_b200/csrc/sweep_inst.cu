@@ -31,6 +31,7 @@ static int launch_any(const SweepLaunch& L, int* ctas_per_sm) {
     switch (L.rows) {
         case 1: return L.uniform ? launch_one<1, true>(L, ctas_per_sm) : launch_one<1, false>(L, ctas_per_sm);
         case 2: return L.uniform ? launch_one<2, true>(L, ctas_per_sm) : launch_one<2, false>(L, ctas_per_sm);
+        case 3: return L.uniform ? launch_one<3, true>(L, ctas_per_sm) : launch_one<3, false>(L, ctas_per_sm);
         default: return L.uniform ? launch_one<4, true>(L, ctas_per_sm) : launch_one<4, false>(L, ctas_per_sm);
     }
 }
