@@ -168,7 +168,7 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
 /* Options.  Every setting gives the same accept/reject sequence as the oracle; settings that change
  * the partition of a row's sum change dE by rounding only (the sums themselves do not depend on the
  * schedule).  Unknown keys and out-of-range values return MC_EINVAL.
- *   "prows"        1|2|4   rows per thread of the sweep kernel; chunk = 256 * prows rows
+ *   "prows"        1|2|3|4 rows per thread of the sweep kernel; chunk = 256 * prows rows
  *                          (default by N: 4 from 32768, 2 from 512, else 1)
  *   "far_cols"     8..65536, multiple of 8: target columns per FAR item (default 256 from N = 32768, else 64)
  *   "pnear"        0..128  worker CTAs that serve only urgent and in-chunk items (default 4)

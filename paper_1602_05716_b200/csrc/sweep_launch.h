@@ -7,7 +7,7 @@ namespace mcb {
 
 struct SweepLaunch {
     PArgs args;
-    int rows;          // rows per consumer thread: 1, 2 or 4
+    int rows;          // rows per consumer thread: 1 to 4
     bool uniform;      // all diameters equal
     int grid;          // CTAs (0: query only)
     cudaStream_t stream;

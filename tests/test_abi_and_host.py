@@ -53,7 +53,7 @@ def test_library_is_sm100a_native_with_bulk_async_copies(lib):
     assert "sm_100a" in out
     sass = subprocess.run(["cuobjdump", "-sass", str(binding._LIBPATH)], capture_output=True, text=True).stdout
     sweep = [blk for blk in sass.split("Function :")[1:] if "k_sweep" in blk.splitlines()[0]]
-    assert len(sweep) == 18, "k_sweep: 3 row counts x 2 diameter paths x 3 pair-distance forms"
+    assert len(sweep) == 24, "k_sweep: 4 row counts x 2 diameter paths x 3 pair-distance forms"
     for blk in sweep:
         assert "UBLKCP" in blk          # cp.async.bulk (TMA unit) staging of the column ring
         assert "SYNCS" in blk           # mbarrier transactions
@@ -164,7 +164,7 @@ def test_reference_arm_prints_one_json_line():
 
 
 @pytest.mark.parametrize("N", [1, 2, 31, 33, 255, 257, 512, 1023, 1025, 4096, 16383, 65536, 100001])
-@pytest.mark.parametrize("rows", [1, 2, 4])
+@pytest.mark.parametrize("rows", [1, 2, 3, 4])
 def test_persistent_kernel_items_cover_every_column_exactly_once(N, rows):
     """Host logic of csrc/persist.cuh: FAR-L + FAR-U + MID + FIX + DIAG partition the N columns of every chunk
     (Eq. 2: each partner enters a trial's sum exactly once)."""

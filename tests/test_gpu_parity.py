@@ -365,7 +365,7 @@ def test_strong_coupling_low_acceptance():
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("opts", [
     # rows per thread / chunk size, item width, near workers, wave rounding, pair-distance form, diameter path
-    {"prows": 1}, {"prows": 2}, {"prows": 4}, {"far_cols": 64}, {"far_cols": 1024}, {"pnear": 0}, {"pnear": 32},
+    {"prows": 1}, {"prows": 2}, {"prows": 3}, {"prows": 4}, {"far_cols": 64}, {"far_cols": 1024}, {"pnear": 0}, {"pnear": 32},
     {"wave": 0}, {"prows": 2, "far_cols": 8, "pnear": 1}, {"debug": 1}, {"form": 1}, {"form": 2},
     {"form": 1, "prows": 1}, {"form": 2, "prows": 4}, {"uniform_path": 0, "form": 2},
     {"diag_split": 1}, {"diag_split": 2}, {"diag_split": 8, "prows": 1}, {"max_ctas": 32}, {"max_ctas": 9, "diag_split": 4}])
