@@ -22,9 +22,18 @@
 namespace mcb {
 
 constexpr int kPThreads = kBulkThreads;        // workers: 8 consumer warps; thread 0 also feeds the column ring
-constexpr int kGroup = 128;                    // rows per published progress step of the chain
-constexpr int kFixCols = 16;                   // columns per FIX item (columns of chunk c-1)
-constexpr int kMidCols = 32;                   // columns per MID item (columns of chunk c-2)
+#ifndef MCB_GROUP
+#define MCB_GROUP 128
+#endif
+#ifndef MCB_FIXCOLS
+#define MCB_FIXCOLS 16
+#endif
+#ifndef MCB_MIDCOLS
+#define MCB_MIDCOLS 32
+#endif
+constexpr int kGroup = MCB_GROUP;              // rows per published progress step of the chain
+constexpr int kFixCols = MCB_FIXCOLS;          // columns per FIX item (columns of chunk c-1)
+constexpr int kMidCols = MCB_MIDCOLS;          // columns per MID item (columns of chunk c-2)
 constexpr int kRing = 4;                       // hand-off ring depth of the chain CTA
 constexpr int kHelpers = 6;
 #ifndef MCB_DRING
