@@ -34,7 +34,10 @@ constexpr int kPThreads = kBulkThreads;        // workers: 8 consumer warps; thr
 constexpr int kGroup = MCB_GROUP;              // rows per published progress step of the chain
 constexpr int kFixCols = MCB_FIXCOLS;          // columns per FIX item (columns of chunk c-1)
 constexpr int kMidCols = MCB_MIDCOLS;          // columns per MID item (columns of chunk c-2)
-constexpr int kRing = 4;                       // hand-off ring depth of the chain CTA
+#ifndef MCB_RING
+#define MCB_RING 3
+#endif
+constexpr int kRing = MCB_RING;                // hand-off ring depth of the chain CTA (measured: 3 beats 4 and 2 at every N)
 constexpr int kHelpers = 6;
 #ifndef MCB_DRING
 #define MCB_DRING 4

@@ -62,11 +62,14 @@ def compare_last_sweep(g, o, tag="", first=0, count=None):
 def lockstep(g, o, sweeps, tag="", every=1, after_sweep=None):
     """Run both chains ``sweeps`` sweeps, comparing after every ``every`` sweeps.  ``after_sweep(done)`` is
     called once both chains are known to be in the same state.  Returns a summary."""
-    worst, flips, done = 0.0, 0, 0
+    import time
+    worst, flips, done, t_oracle = 0.0, 0, 0, 0.0
     while done < sweeps:
         n = min(every, sweeps - done)
         g.mc_sweep(n)
+        t0 = time.perf_counter()
         o.sweep(n)
+        t_oracle += time.perf_counter() - t0      # the CPU-baseline protocol of SURVEY.md 8(d): the oracle's full runs, timed
         done += n
         e, f = compare_last_sweep(g, o, tag=f"{tag} sweep {done - 1}")
         worst = max(worst, e)
@@ -80,7 +83,7 @@ def lockstep(g, o, sweeps, tag="", every=1, after_sweep=None):
                                             f"(max {np.abs(pg - po).max():.3e})")
         if after_sweep is not None:
             after_sweep(done)
-    return {"max_dE_err": worst, "near_tie_flips": flips}
+    return {"max_dE_err": worst, "near_tie_flips": flips, "oracle_seconds": t_oracle}
 
 
 def assert_stats_equal(g, o, flips=0):

@@ -49,7 +49,9 @@ def _full_config_run(w, threads, hist_every_sweep=False):
 
     r = lockstep(g, o, w.sweeps, tag=w.name, after_sweep=sample if hist_every_sweep else None)
     record_margin(w.name, N=w.N, sweeps=w.sweeps, max_dE_err=r["max_dE_err"], near_tie_flips=r["near_tie_flips"],
-                  form=g.mc_get_option("form"), R_over_dmin=w.cavity_R / min(s.diameter for s in w.species))
+                  form=g.mc_get_option("form"), R_over_dmin=w.cavity_R / min(s.diameter for s in w.species),
+                  oracle_threads=threads, oracle_seconds=r["oracle_seconds"],
+                  oracle_pair_evals_per_s=w.sweeps * w.pair_evals_per_sweep / r["oracle_seconds"])
     assert r["max_dE_err"] <= 1e-10
     assert g.sweep_index == w.sweeps == o.sweep_index
     st = g.mc_get_stats()
@@ -101,7 +103,9 @@ def test_config5_n262144_one_full_oracle_sweep_then_invariants():
     e0 = g.mc_energy()
     r = lockstep(g, o, 1, tag=w.name)
     record_margin(w.name, N=w.N, sweeps=1, max_dE_err=r["max_dE_err"], near_tie_flips=r["near_tie_flips"],
-                  form=g.mc_get_option("form"), R_over_dmin=w.cavity_R / min(s.diameter for s in w.species))
+                  form=g.mc_get_option("form"), R_over_dmin=w.cavity_R / min(s.diameter for s in w.species),
+                  oracle_threads=NCPU, oracle_seconds=r["oracle_seconds"],
+                  oracle_pair_evals_per_s=w.pair_evals_per_sweep / r["oracle_seconds"])
     g.mc_sweep(w.sweeps - 1)
     st = g.mc_get_stats()
     e1 = g.mc_energy()
