@@ -38,7 +38,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t xy, zq, hh, lbq, txy, tz, lnu, wall, Dblk, OVold, OVnew, log_dE, log_flags,
-        st, epart, centres, ccount, stage_pos, S1, S2, ovc, nn, sy, gbar, dbg, hcode, hcount, hcursor, hsxy, hszq, hbbox, total;
+        st, epart, centres, ccount, stage_pos, S1, S2, ovc, nn, sy, gbar, uc, dbg, hcode, hcount, hcursor, hsxy, hszq, hbbox, total;
 };
 
 int padded(int64_t N) { return (int)((N + kTile - 1) / kTile * kTile); }
@@ -57,6 +57,7 @@ Layout make_layout(int64_t N) {
     L.S1 = take(Np * 8); L.S2 = take(Np * 8); L.ovc = take(Np * 4); L.nn = take(Np * 8);
     L.sy = take((size_t)2 * (kSyHdr + 4 * (Np / 256 + 1)) * 4);   // live words + snapshot of the last completed sweep
     L.gbar = take(256);
+    L.uc = take(((size_t)(Np / 256 + 2) * (kChunkMax / kGroup + 1) + 16) * 4);   // urgent_units() at the smallest chunk size, rounded up
     L.dbg = take(kDbgWords * 8);
     L.hcode = take(Np * 4); L.hcount = take((size_t)kCells * 4); L.hcursor = take((size_t)kCells * 4);
     L.hsxy = take(Np * 16); L.hszq = take(Np * 16); L.hbbox = take((Np / 256 + 1) * 4 * 6 * 8);
@@ -140,6 +141,7 @@ int launch_sweep(mc_handle* h, cudaStream_t s, int nsweeps) {
     a.nsweeps = nsweeps;
     a.sy = h->p.sy;
     a.gbar = (int*)(h->ws + h->L.gbar);
+    a.uc = (int*)(h->ws + h->L.uc);
     a.dbg = h->debug ? (long long*)(h->ws + h->L.dbg) : nullptr;
     if (a.dbg) CUDA_TRY(cudaMemsetAsync(a.dbg, 0, kDbgWords * 8, s));
     L.grid = h->pgrid;
@@ -154,6 +156,7 @@ constexpr int64_t kMaxSweepsPerLaunch = 1024;   // keeps a single launch bounded
 int reset_scheduling(mc_handle* h) {
     CUDA_TRY(cudaMemsetAsync(h->p.sy, 0, (size_t)h->p.sy_n * 4, h->stream));
     CUDA_TRY(cudaMemsetAsync(h->ws + h->L.gbar, 0, 256, h->stream));
+    CUDA_TRY(cudaMemsetAsync(h->ws + h->L.uc, 0, ((size_t)(h->p.Np / 256 + 2) * (kChunkMax / kGroup + 1) + 16) * 4, h->stream));
     return MC_OK;
 }
 

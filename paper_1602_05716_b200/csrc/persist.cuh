@@ -67,6 +67,7 @@ struct PArgs {
     int* sy;          // [kSyHdr + 3 * nchunks]: header, far_done, diag_done, fix_done; all zero at launch and again at exit
     int* gbar;        // grid barrier: [0] arrivals, [32] generation
     long long* dbg;   // [16] diagnostic cycle counters (see mc_debug_counters), may be null
+    int* uc;          // claim counters of the urgent release units (urgent_units() ints, zero between sweeps), see fetch_item
 };
 
 __host__ __device__ inline int chunk_rows(int Np, int C, int c) { return min(C, Np - c * C); }
@@ -85,6 +86,17 @@ __host__ __device__ inline int farL_cols(int C, int c) { return c >= 3 ? (c - 2)
 // urgent items of chunk c: MID (columns of chunk c-2, c >= 2) then FIX (columns of chunk c-1, c >= 1)
 __host__ __device__ inline int urgent_items(int C, int c) {
     return (c >= 2 ? C / kMidCols : 0) + (c >= 1 ? C / kFixCols : 0);
+}
+// The urgent items are claimed by RELEASE UNIT: all items of a unit become claimable at the same moment -- MID(c), the
+// C / kMidCols items over the columns of chunk c-2, when the chain has finished chunk c-2; FIX(c, g), the
+// kGroup / kFixCols items over group g of chunk c-1, when the chain has published that group -- so one atomicAdd on the
+// unit's counter hands out its items in parallel and can never reach into work that does not exist yet.  (Round 1 and
+// the first half of round 2 took urgent tickets in order with a compare-and-swap: the eight items of a group were
+// claimed one round trip after the other, 3.5 us for the last one at every chunk boundary.)
+// Units in release order: chunk 1: FIX groups 0..GPC-1;  chunk c >= 2: MID(c), then FIX groups 0..GPC-1.
+__host__ __device__ inline int urgent_units(int C, int nchunks) {
+    const int GPC = C / kGroup;
+    return nchunks >= 2 ? GPC + (nchunks - 2) * (GPC + 1) : 0;
 }
 __host__ __device__ inline int farU_cols(int Np, int C, int c) { return Np - (c * C + chunk_rows(Np, C, c)); }
 __host__ __device__ inline int probe_cols(int Np, int C, int c) { return Np - chunk_rows(Np, C, c); }
@@ -753,6 +765,7 @@ struct Cursor {
 };
 struct Cursors {
     Cursor l, u, d;
+    int uunit;      // first urgent release unit this CTA has not seen exhausted
 };
 
 template <int Q>
@@ -809,7 +822,7 @@ __device__ __forceinline__ int ld_relaxed(const int* p) {
 
 static __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near, int* item) {
     const int C = a.C, GPC = C / kGroup, nfix = C / kFixCols, nmid = C / kMidCols;
-    const int total_urgent = a.nchunks >= 2 ? nfix + (a.nchunks - 2) * (nfix + nmid) : 0;
+    const int total_units = urgent_units(C, a.nchunks), nper = kGroup / kFixCols;
     int* sy = a.sy;
     for (unsigned it = 1;; ++it) {
         // no time limit of its own: leaves when another wait gave up -- through an exit ITEM, not by exiting: the
@@ -817,34 +830,38 @@ static __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, boo
         if ((it & 1023u) == 0u && *(volatile int*)(sy + kSyAbort) != 0) { item[0] = kItemExit; return; }
         // one round trip: five independent loads
         const int tl = ld_relaxed(sy + kSyTicket), tu = ld_relaxed(sy + kSyTicketU), td = ld_relaxed(sy + kSyDTicket);
-        const int u = ld_relaxed(sy + kSyUTicket), groups = ld_acquire(sy + kSyGroups);   // acquire: what the chain published
+        const int hint = ld_relaxed(sy + kSyUTicket), groups = ld_acquire(sy + kSyGroups);   // acquire: what the chain published
         bool got = false, l_done = true, u_done = true, d_done = false;
         if (a.mode == 1) {
             got = try_queue<QU>(a, cur.u, tu, groups, item, u_done);
             if (!got) item[0] = kItemExit;
             return;
         }
-        if (!got && u < total_urgent) {
-            // urgent ticket u -> chunk c, MID item j (columns of chunk c-2) or FIX item j (columns of chunk c-1)
-            int c = 1, j = u, mid = 0;
-            if (u >= nfix) {
-                c = 2 + (u - nfix) / (nfix + nmid);
-                j = (u - nfix) % (nfix + nmid);
-                mid = j < nmid ? 1 : 0;
-                if (!mid) j -= nmid;
-            }
-            const int need = mid ? (c - 1) * GPC : (c - 1) * GPC + (j * kFixCols) / kGroup + 1;
-            if (groups >= need) {
-                if (atomicCAS(sy + kSyUTicket, u, u + 1) != u) continue;
-                item[0] = mid ? kItemMid : kItemFix; item[1] = c; item[2] = j;
+        // urgent items: walk the release units from the first one not known to be exhausted (this CTA's own
+        // knowledge or the shared hint), stop at the first unit the chain has not released yet
+        int k = max(cur.uunit, hint);
+        while (k < total_units) {
+            int c, g, mid;                         // unit k -> chunk c, MID unit or FIX group g
+            if (k < GPC) { c = 1; g = k; mid = 0; }
+            else { c = 2 + (k - GPC) / (GPC + 1); g = (k - GPC) % (GPC + 1) - 1; mid = g < 0 ? 1 : 0; }
+            const int need = mid ? (c - 1) * GPC : (c - 1) * GPC + g + 1;
+            if (groups < need) break;
+            const int size = mid ? nmid : nper;
+            const int v = atomicAdd(a.uc + k, 1);
+            if (v < size) {
+                item[0] = mid ? kItemMid : kItemFix; item[1] = c; item[2] = mid ? v : g * nper + v;
                 got = true;
+                if (v == size - 1) atomicMax(sy + kSyUTicket, k + 1);     // the hint for everybody else
+                break;
             }
+            ++k;
         }
+        cur.uunit = k;
         if (!got) got = try_queue<QD>(a, cur.d, td, groups, item, d_done);
         if (!got && !near) got = try_queue<QL>(a, cur.l, tl, groups, item, l_done);
         if (!got && !near) got = try_queue<QU>(a, cur.u, tu, groups, item, u_done);
         if (got) return;
-        if (l_done && u_done && d_done && u >= total_urgent) { item[0] = kItemExit; return; }
+        if (l_done && u_done && d_done && k >= total_units) { item[0] = kItemExit; return; }
         __nanosleep(near ? 400 : 200);
     }
 }
@@ -920,7 +937,7 @@ __device__ __forceinline__ void worker_sweep(const PArgs& a, PShared& sh, unsign
     const int tid = threadIdx.x, warp = tid >> 5;
     const Params& p = a.p;
     const int C = a.C;
-    Cursors cur{{0, 0, -1}, {0, 0, -1}, {0, 0, -1}};
+    Cursors cur{{0, 0, -1}, {0, 0, -1}, {0, 0, -1}, 0};
     if (a.dbg && blockIdx.x == 1 && tid == 0) a.dbg[16 + 3 * 300 + 40] = (long long)global_ns();
     const bool near = (int)blockIdx.x <= a.nnear;
     for (;;) {
@@ -1063,6 +1080,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
                 a.sy[p.sy_n + j] = a.sy[j];
                 if (last || j != kSyChainSm) a.sy[j] = 0;
             }
+            for (int j = tid; j < urgent_units(a.C, a.nchunks); j += kPThreads) a.uc[j] = 0;
         }
     }
 }
