@@ -187,6 +187,8 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
  *   "diag_split"   0|1|2|4|8  warps that share one 32 x 32 in-chunk unit of the sweep kernel, each taking a part of
  *                          its columns -- the multi-thread-per-particle scheme of PAPER.md:243-245 for systems too
  *                          small to fill the device (0 = by N: 8 up to 2048 ions, 4 up to 8192, 2 up to 32768, else 1)
+ *   "fix_cols"     0|4|8|16 columns per urgent item over the chunk just finished (0 = by N: 16 from N = 32768, else 4:
+ *                          where the chain paces the sweep, many short items finish sooner than few long ones)
  *   "max_ctas"     0..4096 upper limit on the CTAs of the sweep kernel (0 = two per SM, the default for large
  *                          systems; small systems synchronise faster on a smaller grid)
  *   "energy_rows"  4|6|8   rows per thread of the from-scratch energy kernel

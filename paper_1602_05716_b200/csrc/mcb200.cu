@@ -81,6 +81,7 @@ struct mc_handle {
     int num_sms = 148;
     int prows = 4;           // rows per consumer thread of the sweep kernel (chunk = 256 * prows)
     int pfarcols = 256;      // columns per FAR item of the sweep kernel
+    int fixcols = 0;         // columns per FIX item of the sweep kernel (0: by N)
     int dsplit = 0;          // warps per DIAG unit of the sweep kernel (0: by N)
     int erows = 4;           // rows per thread of k_energy (Gram form)
     int hist_slices = 64;   // column slices (grid.y) of k_hist
@@ -138,6 +139,7 @@ int launch_sweep(mc_handle* h, cudaStream_t s, int nsweeps) {
     a.mode = h->pmode;
     a.nfar = h->pwave ? std::max(1, h->pgrid - 2 - a.nnear) : 0;
     a.dsplit = h->dsplit > 0 ? h->dsplit : (a.p.Np <= 2048 ? 8 : a.p.Np <= 8192 ? 4 : a.p.Np <= 32768 ? 2 : 1);
+    a.fixcols = h->fixcols > 0 ? h->fixcols : (a.p.Np >= 32768 ? 16 : 4);
     a.nsweeps = nsweeps;
     a.sy = h->p.sy;
     a.gbar = (int*)(h->ws + h->L.gbar);
@@ -541,6 +543,9 @@ int mc_set_option(mc_handle* h, const char* key, int64_t value) {
     } else if (!std::strcmp(key, "pnear")) {
         if (value < 0 || value > 128) return fail(MC_EINVAL, "pnear must be in 0..128");
         h->pnear = (int)value;
+    } else if (!std::strcmp(key, "fix_cols")) {
+        if (value != 0 && value != 4 && value != 8 && value != 16) return fail(MC_EINVAL, "fix_cols must be 0 (by N), 4, 8 or 16");
+        h->fixcols = (int)value;
     } else if (!std::strcmp(key, "diag_split")) {
         if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) return fail(MC_EINVAL, "diag_split must be 0 (by N), 1, 2, 4 or 8");
         h->dsplit = (int)value;
@@ -598,6 +603,7 @@ int mc_get_option(mc_handle* h, const char* key, int64_t* value_host) {
     else if (!std::strcmp(key, "wave")) *value_host = h->pwave ? 1 : 0;
     else if (!std::strcmp(key, "max_ctas")) *value_host = h->max_ctas;
     else if (!std::strcmp(key, "diag_split")) *value_host = h->dsplit;
+    else if (!std::strcmp(key, "fix_cols")) *value_host = h->fixcols;
     else if (!std::strcmp(key, "form")) *value_host = h->form;
     else if (!std::strcmp(key, "form_auto")) *value_host = h->form_auto;
     else if (!std::strcmp(key, "position_bits")) *value_host = h->p.pos_bits;

@@ -32,7 +32,8 @@ constexpr int kPThreads = kBulkThreads;        // workers: 8 consumer warps; thr
 #define MCB_MIDCOLS 32
 #endif
 constexpr int kGroup = MCB_GROUP;              // rows per published progress step of the chain
-constexpr int kFixCols = MCB_FIXCOLS;          // columns per FIX item (columns of chunk c-1)
+constexpr int kFixCols = MCB_FIXCOLS;          // columns per FIX item (columns of chunk c-1): the default for large systems;
+                                               // PArgs::fixcols is what a launch uses (4 where the chain paces the sweep)
 constexpr int kMidCols = MCB_MIDCOLS;          // columns per MID item (columns of chunk c-2)
 #ifndef MCB_RING
 #define MCB_RING 3
@@ -63,6 +64,7 @@ struct PArgs {
     int mode;         // 0 normal; 1 throughput probe: no chain, every CTA runs QU items over all columns but the chunk's own;
                       // 2 watchdog test: the deciding warp never runs, so the sweep stalls
     int dsplit;       // warps that share one DIAG unit: 1, 2, 4 or 8
+    int fixcols;      // columns per FIX item: 4, 8 or 16
     int nsweeps;      // sweeps this launch runs (a1-a4 each), separated by grid-wide barriers
     int* sy;          // [kSyHdr + 3 * nchunks]: header, far_done, diag_done, fix_done; all zero at launch and again at exit
     int* gbar;        // grid barrier: [0] arrivals, [32] generation
@@ -84,8 +86,8 @@ __host__ __device__ inline int far_slices(int ncols, int farcols, int nfar) {
 // finished chunk c-3), U = after chunk c (sweep-start positions, never blocked)
 __host__ __device__ inline int farL_cols(int C, int c) { return c >= 3 ? (c - 2) * C : 0; }
 // urgent items of chunk c: MID (columns of chunk c-2, c >= 2) then FIX (columns of chunk c-1, c >= 1)
-__host__ __device__ inline int urgent_items(int C, int c) {
-    return (c >= 2 ? C / kMidCols : 0) + (c >= 1 ? C / kFixCols : 0);
+__host__ __device__ inline int urgent_items(int C, int c, int fixcols = kFixCols) {
+    return (c >= 2 ? C / kMidCols : 0) + (c >= 1 ? C / fixcols : 0);
 }
 // The urgent items are claimed by RELEASE UNIT: all items of a unit become claimable at the same moment -- MID(c), the
 // C / kMidCols items over the columns of chunk c-2, when the chain has finished chunk c-2; FIX(c, g), the
@@ -495,7 +497,7 @@ __device__ __forceinline__ void chain_helper_tile(const PArgs& a, PShared& sh, c
         const long long t0 = clock64();
         spin_until_ge(wd, sy_far_done(a) + c, far_items(a.p.Np, C, a.farcols, a.nfar, c));
         const long long t1 = clock64();
-        if (c > 0) spin_until_ge(wd, sy_fix_done(a) + c, urgent_items(C, c));
+        if (c > 0) spin_until_ge(wd, sy_fix_done(a) + c, urgent_items(C, c, a.fixcols));
         if (t == 0 && lane == 0 && a.dbg) {
             a.dbg[3] += t1 - t0; a.dbg[4] += clock64() - t1;
             if (c < 300) a.dbg[16 + 3 * c] = (long long)global_ns();   // inputs of chunk c complete
@@ -821,8 +823,8 @@ __device__ __forceinline__ int ld_relaxed(const int* p) {
 }
 
 static __device__ __noinline__ void fetch_item(const PArgs& a, Cursors& cur, bool near, int* item) {
-    const int C = a.C, GPC = C / kGroup, nfix = C / kFixCols, nmid = C / kMidCols;
-    const int total_units = urgent_units(C, a.nchunks), nper = kGroup / kFixCols;
+    const int C = a.C, GPC = C / kGroup, nmid = C / kMidCols;
+    const int total_units = urgent_units(C, a.nchunks), nper = kGroup / a.fixcols;
     int* sy = a.sy;
     for (unsigned it = 1;; ++it) {
         // no time limit of its own: leaves when another wait gave up -- through an exit ITEM, not by exiting: the
@@ -974,7 +976,7 @@ __device__ __forceinline__ void worker_sweep(const PArgs& a, PShared& sh, unsign
                 v0 = slice_bound(ncols, nf, k); v1 = slice_bound(ncols, nf, k + 1);
                 g0 = probe ? row0 : cb; g1 = probe ? row0 + nrows : cb;
             } else {
-                const int w = type == kItemMid ? kMidCols : kFixCols;
+                const int w = type == kItemMid ? kMidCols : a.fixcols;
                 cb = row0 - (type == kItemMid ? 2 : 1) * C + k * w;
                 g0 = g1 = cb; v0 = 0; v1 = w;
             }
@@ -1070,7 +1072,7 @@ __global__ void __launch_bounds__(kPThreads, 2) k_sweep(const PArgs a) {
                 for (int c = tid; c < a.nchunks; c += kPThreads) {
                     bad |= a.sy[kSyHdr + c] != far_items(p.Np, a.C, a.farcols, a.nfar, c);
                     bad |= a.sy[kSyHdr + a.nchunks + c] != diag_items(chunk_rows(p.Np, a.C, c), a.dsplit);
-                    bad |= a.sy[kSyHdr + 2 * a.nchunks + c] != urgent_items(a.C, c);
+                    bad |= a.sy[kSyHdr + 2 * a.nchunks + c] != urgent_items(a.C, c, a.fixcols);
                 }
                 if (__syncthreads_or(bad) && tid == 0) p.st->sched_mismatch += 1;
             }

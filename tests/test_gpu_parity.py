@@ -372,7 +372,7 @@ def test_strong_coupling_low_acceptance():
     {"prows": 1}, {"prows": 2}, {"prows": 3}, {"prows": 4}, {"far_cols": 64}, {"far_cols": 1024}, {"pnear": 0}, {"pnear": 32},
     {"wave": 0}, {"prows": 2, "far_cols": 8, "pnear": 1}, {"debug": 1}, {"form": 1}, {"form": 2},
     {"form": 1, "prows": 1}, {"form": 2, "prows": 4}, {"uniform_path": 0, "form": 2},
-    {"diag_split": 1}, {"diag_split": 2}, {"diag_split": 8, "prows": 1}, {"max_ctas": 32}, {"max_ctas": 9, "diag_split": 4}])
+    {"fix_cols": 4}, {"fix_cols": 8, "prows": 4}, {"fix_cols": 16}, {"diag_split": 1}, {"diag_split": 2}, {"diag_split": 8, "prows": 1}, {"max_ctas": 32}, {"max_ctas": 9, "diag_split": 4}])
 @pytest.mark.parametrize("base", [2, 3])      # two diameters / equal diameters (the specialised path)
 def test_every_launch_configuration_gives_the_same_chain(opts, base):
     w = W.scaled(W.CONFIGS[base], 2500)
@@ -437,7 +437,8 @@ def test_soak_completion_counters_after_every_sweep(N, pnear):
             nt = [min(C_, Np - c * C_) // 32 for c in range(nchunks)]
             split = {True: 8, False: 4 if Np <= 8192 else 2 if Np <= 32768 else 1}[Np <= 2048]   # warps per DIAG unit, by N
             want_diag = np.array([(t * t * split + 7) // 8 for t in nt])
-            want_fix = np.array([(C_ // 32 if c >= 2 else 0) + (C_ // 16 if c >= 1 else 0) for c in range(nchunks)])
+            fixc = 16 if Np >= 32768 else 4                      # columns per FIX item, by N
+            want_fix = np.array([(C_ // 32 if c >= 2 else 0) + (C_ // fixc if c >= 1 else 0) for c in range(nchunks)])
             assert np.array_equal(diag, want_diag) and np.array_equal(fix, want_fix)
             want = (far.copy(), want_diag, want_fix)
             assert far.sum() + want_diag.sum() + want_fix.sum() > 0
@@ -462,6 +463,7 @@ def test_far_item_count_matches_the_host_plan():
         pos, q, d = w.arrays()
         g = MCSystem(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 1)
         g.mc_set_option("diag_split", 1)                 # the host plan counts one warp per in-chunk unit
+        g.mc_set_option("fix_cols", 16)                  # ... and 16 columns per FIX item
         g.mc_sweep(1)
         g.synchronize()
         rows = g.mc_get_option("prows")
