@@ -155,7 +155,8 @@ int mc_debug_counters(mc_handle* h, int64_t* out16_host);
  * chunk of 256 * rows_per_thread rows of an N-particle system, the FAR-L, FAR-U, MID, FIX and DIAG
  * items exactly as the kernel slices them (far_cols = target columns per FAR item, far_workers = the
  * number the item counts are rounded to, 0 = no rounding) and verifies that every column is covered
- * exactly once per chunk.  out4_host = {items, violations, widest item in columns, urgent items}. */
+ * exactly once per chunk, and that the urgent items' release units hand out every MID and FIX item exactly
+ * once, in the order in which the chain releases them (for 4, 8 and 16 columns per FIX item).  out4_host = {items, violations, widest item in columns, urgent items}. */
 int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers, int64_t* out4_host);
 
 /* Diagnostics: copies the first n ints of the sweep kernel's scheduling state -- W = 256 + 4 (N / 256 + 1) live

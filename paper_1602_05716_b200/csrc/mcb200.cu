@@ -662,6 +662,31 @@ int mc_plan_check(int64_t N, int rows_per_thread, int far_cols, int far_workers,
         items += diag_items(nrows, 1);
         for (int k = 0; k < Np / 8; ++k) violations += cover[k] != 1;
     }
+    // the urgent items by release unit, as fetch_item (persist.cuh) hands them out: every (chunk, MID item) and
+    // (chunk, FIX item) exactly once, in non-decreasing order of the chain progress that releases them
+    for (int fixcols : {4, 8, 16}) {
+        const int GPC = C / kGroup, nper = kGroup / fixcols, nmid = C / kMidCols, nfix = C / fixcols;
+        std::vector<int> seen((size_t)nchunks * (nmid + nfix), 0);
+        int last_need = 0;
+        const int units = urgent_units(C, nchunks);
+        for (int k = 0; k < units; ++k) {
+            int c, g, mid;
+            if (k < GPC) { c = 1; g = k; mid = 0; }
+            else { c = 2 + (k - GPC) / (GPC + 1); g = (k - GPC) % (GPC + 1) - 1; mid = g < 0 ? 1 : 0; }
+            const int need = mid ? (c - 1) * GPC : (c - 1) * GPC + g + 1;
+            if (need < last_need || c >= nchunks) ++violations;
+            last_need = need;
+            for (int v = 0; v < (mid ? nmid : nper); ++v) {
+                const int j = mid ? v : g * nper + v;
+                if (c < nchunks) ++seen[(size_t)c * (nmid + nfix) + (mid ? j : nmid + j)];
+            }
+        }
+        for (int c = 0; c < nchunks; ++c)
+            for (int j = 0; j < nmid + nfix; ++j) {
+                const int want = j < nmid ? (c >= 2 ? 1 : 0) : (c >= 1 ? 1 : 0);
+                violations += seen[(size_t)c * (nmid + nfix) + j] != want;
+            }
+    }
     out4_host[0] = items; out4_host[1] = violations; out4_host[2] = max_item_cols; out4_host[3] = urgent;
     return MC_OK;
 }

@@ -726,3 +726,20 @@ def test_long_run_mean_energy_and_g_of_r_agree_with_independent_oracle_chain():
     m1, s1 = _blocked_mean_se(cg[:, 0, 2]); m2, s2 = _blocked_mean_se(cg[:, 1, 2])
     assert (m1 - m2) / np.hypot(s1, s2) > 6.0                  # unlike ions sit closer than like ions
     record_margin("long_run_statistics", energy_z=abs(mg - mo) / np.hypot(sg, so), g_of_r_zmax=zmax)
+
+
+def test_more_sweeps_than_one_launch_holds():
+    """mc_sweep(n) runs at most 1024 sweeps per launch: n = 1030 is two launches and must equal 1000 + 30."""
+    from paper_1602_05716_b200.binding import MCSystem
+    w = W.scaled(W.CONFIGS[0], 300)
+    pos, q, d = w.arrays()
+    a = MCSystem(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 9)
+    b = MCSystem(pos, q, d, w.cavity_R, w.bjerrum, w.max_disp, 9)
+    a.mc_sweep(1030)
+    b.mc_sweep(1000); b.mc_sweep(30)
+    assert a.sweep_index == b.sweep_index == 1030
+    assert np.array_equal(a.positions, b.positions)
+    assert a.mc_get_stats() == b.mc_get_stats()
+    e = a.mc_energy()
+    assert abs(a.mc_get_stats()["E_running"] - e) < 1e-8 * max(1.0, abs(e))
+    assert hard_constraints_ok(a.positions, d, w.cavity_R)
