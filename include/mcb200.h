@@ -170,8 +170,9 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
  * the partition of a row's sum change dE by rounding only (the sums themselves do not depend on the
  * schedule).  Unknown keys and out-of-range values return MC_EINVAL.
  *   "prows"        1|2|3|4 rows per thread of the sweep kernel; chunk = 256 * prows rows
- *                          (default by N: 4 from 32768, 2 from 512, else 1)
- *   "far_cols"     8..65536, multiple of 8: target columns per FAR item (default 256 from N = 32768, else 64)
+ *                          (default by N: 3 from 36864, 2 from 512, else 1)
+ *   "far_cols"     8..65536, multiple of 8: target columns per FAR item (default by N: 64 below 36864, 128 below 53248,
+ *                          256 below 114688, else 384)
  *   "pnear"        0..128  worker CTAs that serve only urgent and in-chunk items (default 4)
  *   "wave"         0|1     round a chunk's FAR items to a multiple of the FAR workers (default 1)
  *   "form"         -1|0|1|2  pair-distance form (persist.cuh): -1 = by geometry (default): 0 GRAM if
@@ -188,7 +189,7 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
  *   "diag_split"   0|1|2|4|8  warps that share one 32 x 32 in-chunk unit of the sweep kernel, each taking a part of
  *                          its columns -- the multi-thread-per-particle scheme of PAPER.md:243-245 for systems too
  *                          small to fill the device (0 = by N: 8 up to 2048 ions, 4 up to 8192, 2 up to 32768, else 1)
- *   "fix_cols"     0|4|8|16 columns per urgent item over the chunk just finished (0 = by N: 16 from N = 32768, else 4:
+ *   "fix_cols"     0|4|8|16 columns per urgent item over the chunk just finished (0 = by N: 16 from N = 53248, 8 from 36864, else 4:
  *                          where the chain paces the sweep, many short items finish sooner than few long ones)
  *   "max_ctas"     0..4096 upper limit on the CTAs of the sweep kernel (0 = two per SM, the default for large
  *                          systems; small systems synchronise faster on a smaller grid)

@@ -139,7 +139,7 @@ int launch_sweep(mc_handle* h, cudaStream_t s, int nsweeps) {
     a.mode = h->pmode;
     a.nfar = h->pwave ? std::max(1, h->pgrid - 2 - a.nnear) : 0;
     a.dsplit = h->dsplit > 0 ? h->dsplit : (a.p.Np <= 2048 ? 8 : a.p.Np <= 8192 ? 4 : a.p.Np <= 32768 ? 2 : 1);
-    a.fixcols = h->fixcols > 0 ? h->fixcols : (a.p.Np >= 32768 ? 16 : 4);
+    a.fixcols = h->fixcols > 0 ? h->fixcols : (a.p.Np >= 53248 ? 16 : a.p.Np >= 36864 ? 8 : 4);
     a.nsweeps = nsweeps;
     a.sy = h->p.sy;
     a.gbar = (int*)(h->ws + h->L.gbar);
@@ -245,10 +245,11 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     p.nn = (double*)(w + L.nn);
     p.S1 = (long long*)(w + L.S1); p.S2 = (long long*)(w + L.S2); p.ovc = (int*)(w + L.ovc);
     p.sy_n = kSyHdr + 4 * (p.Np / 256 + 1);   // header + per-chunk counters
-    // measured on B200: 1024-row chunks and 256-column items pay only when the pair work fills the
-    // device; below that the chain paces the sweep and shorter chunks and items keep its inputs ahead of it
-    h->prows = p.Np >= 32768 ? 4 : (p.Np >= 512 ? 2 : 1);
-    h->pfarcols = p.Np >= 32768 ? 256 : 64;
+    // measured on B200 (DESIGN.md sections 7 and 9, option sweeps at N = 512 ... 262144): long chunks and wide items pay
+    // only when the pair work fills the device; below that the chain paces the sweep and shorter chunks and items keep
+    // its inputs ahead of it
+    h->prows = p.Np >= 36864 ? 3 : (p.Np >= 512 ? 2 : 1);
+    h->pfarcols = p.Np >= 114688 ? 384 : p.Np >= 53248 ? 256 : p.Np >= 36864 ? 128 : 64;
     p.R = cavity_R; p.lB = bjerrum_length; p.max_disp = max_disp; p.seed = seed;
     p.wait_limit_ns = 2000000000ull;
     p.pos_bits = 64;

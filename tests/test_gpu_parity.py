@@ -437,7 +437,7 @@ def test_soak_completion_counters_after_every_sweep(N, pnear):
             nt = [min(C_, Np - c * C_) // 32 for c in range(nchunks)]
             split = {True: 8, False: 4 if Np <= 8192 else 2 if Np <= 32768 else 1}[Np <= 2048]   # warps per DIAG unit, by N
             want_diag = np.array([(t * t * split + 7) // 8 for t in nt])
-            fixc = 16 if Np >= 32768 else 4                      # columns per FIX item, by N
+            fixc = 16 if Np >= 53248 else 8 if Np >= 36864 else 4   # columns per FIX item, by N
             want_fix = np.array([(C_ // 32 if c >= 2 else 0) + (C_ // fixc if c >= 1 else 0) for c in range(nchunks)])
             assert np.array_equal(diag, want_diag) and np.array_equal(fix, want_fix)
             want = (far.copy(), want_diag, want_fix)
