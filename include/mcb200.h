@@ -173,7 +173,7 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
  *                          (default by N: 3 from 36864, 2 from 512, else 1)
  *   "far_cols"     8..65536, multiple of 8: target columns per FAR item (default by N: 64 below 36864, 128 below 53248,
  *                          256 below 114688, else 384)
- *   "pnear"        0..128  worker CTAs that serve only urgent and in-chunk items (default 4)
+ *   "pnear"        0..128  worker CTAs that serve only urgent and in-chunk items (default 4 from N = 36864, else 8)
  *   "wave"         0|1     round a chunk's FAR items to a multiple of the FAR workers (default 1)
  *   "form"         -1|0|1|2  pair-distance form (persist.cuh): -1 = by geometry (default): 0 GRAM if
  *                          cavity_R / d_min <= 128, else 1 DIFFW if max_disp / d_min <= 64, else 2 CANON;
@@ -188,7 +188,7 @@ int mc_debug_peek(mc_handle* h, int32_t* out_host, int n);
  *                          raise it under a profiler, a sanitizer or GPU time-slicing)
  *   "diag_split"   0|1|2|4|8  warps that share one 32 x 32 in-chunk unit of the sweep kernel, each taking a part of
  *                          its columns -- the multi-thread-per-particle scheme of PAPER.md:243-245 for systems too
- *                          small to fill the device (0 = by N: 8 up to 2048 ions, 4 up to 8192, 2 up to 32768, else 1)
+ *                          small to fill the device (0 = by N: 4 up to 768 ions, 2 up to 6144, else 1)
  *   "fix_cols"     0|4|8|16 columns per urgent item over the chunk just finished (0 = by N: 16 from N = 53248, 8 from 36864, else 4:
  *                          where the chain paces the sweep, many short items finish sooner than few long ones)
  *   "max_ctas"     0..4096 upper limit on the CTAs of the sweep kernel (0 = two per SM, the default for large

@@ -138,7 +138,7 @@ int launch_sweep(mc_handle* h, cudaStream_t s, int nsweeps) {
     a.farcols = h->pfarcols;
     a.mode = h->pmode;
     a.nfar = h->pwave ? std::max(1, h->pgrid - 2 - a.nnear) : 0;
-    a.dsplit = h->dsplit > 0 ? h->dsplit : (a.p.Np <= 2048 ? 8 : a.p.Np <= 8192 ? 4 : a.p.Np <= 32768 ? 2 : 1);
+    a.dsplit = h->dsplit > 0 ? h->dsplit : (a.p.Np <= 768 ? 4 : a.p.Np <= 6144 ? 2 : 1);
     a.fixcols = h->fixcols > 0 ? h->fixcols : (a.p.Np >= 53248 ? 16 : a.p.Np >= 36864 ? 8 : 4);
     a.nsweeps = nsweeps;
     a.sy = h->p.sy;
@@ -250,6 +250,7 @@ int mc_init(mc_handle** out, int64_t N, const double* pos_dev, const double* cha
     // its inputs ahead of it
     h->prows = p.Np >= 36864 ? 3 : (p.Np >= 512 ? 2 : 1);
     h->pfarcols = p.Np >= 114688 ? 384 : p.Np >= 53248 ? 256 : p.Np >= 36864 ? 128 : 64;
+    h->pnear = p.Np >= 36864 ? 4 : 8;
     p.R = cavity_R; p.lB = bjerrum_length; p.max_disp = max_disp; p.seed = seed;
     p.wait_limit_ns = 2000000000ull;
     p.pos_bits = 64;

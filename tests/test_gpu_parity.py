@@ -435,7 +435,7 @@ def test_soak_completion_counters_after_every_sweep(N, pnear):
             # the plan: diag items = ceil(nt^2 / 8); urgent = C/32 (c >= 2) + C/16 (c >= 1); far from the first sweep,
             # cross-checked against the total mc_plan_check reports
             nt = [min(C_, Np - c * C_) // 32 for c in range(nchunks)]
-            split = {True: 8, False: 4 if Np <= 8192 else 2 if Np <= 32768 else 1}[Np <= 2048]   # warps per DIAG unit, by N
+            split = 4 if Np <= 768 else 2 if Np <= 6144 else 1   # warps per DIAG unit, by N
             want_diag = np.array([(t * t * split + 7) // 8 for t in nt])
             fixc = 16 if Np >= 53248 else 8 if Np >= 36864 else 4   # columns per FIX item, by N
             want_fix = np.array([(C_ // 32 if c >= 2 else 0) + (C_ // fixc if c >= 1 else 0) for c in range(nchunks)])
