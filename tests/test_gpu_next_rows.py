@@ -177,3 +177,15 @@ def test_parallel_reduction_comparison_kernel_runs_the_same_chain(base, N):
     assert g.sweep_index == 6
     assert g.mc_get_launch_count() - l0 >= 3 * w.N          # three of the six sweeps took N launches each
     assert abs(g.mc_get_stats()["E_running"] - g.mc_energy()) <= 1e-9 * abs(g.mc_energy())
+
+
+def test_selfcheck_and_tune_scripts_run():
+    """The two user-facing scripts of the package: the oracle-free invariants of a small run, and the option sweep
+    behind the scheduling defaults (here on a tiny grid of settings)."""
+    from paper_1602_05716_b200 import selfcheck, tune
+    r = selfcheck.run(n=1200, sweeps=2)
+    assert r["N"] == 1200 and r["accepted"] > 0
+    t = tune.run(n=3000, workload=3, sweeps=2, top=3, full=False)
+    assert t["N"] == 3000 and len(t["best"]) == 3
+    assert t["best"][0]["us_per_sweep"] <= t["best"][-1]["us_per_sweep"]
+    assert t["best"][0]["us_per_sweep"] < 3.0 * t["defaults_us_per_sweep"]
