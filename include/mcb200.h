@@ -94,6 +94,22 @@ int mc_energy(mc_handle* h, double* E_host);
 /* Same energy, left in device memory (E_dev, one double); enqueued, no host sync. */
 int mc_energy_dev(mc_handle* h, double* E_dev);
 
+/* The same energy for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no handle, no workspace, and the call itself calls no cudaMalloc, cudaFree
+ * or allocating library routine.  E_dev (device, one double) := bjerrum_length * sum_{i<j} q_i q_j / r_ij (PAPER.md:60-63
+ * Eq. 2's pair term summed over all pairs; the energy that is monitored) of the N ions at pos_dev
+ * ([3][N], device) with charges charges_dev ([N], device), on the CURRENT device, enqueued on `stream` (a cudaStream_t,
+ * NULL = the default stream), no host sync.  Inputs are not validated.  The per-CTA partial sums go through a static
+ * __device__ array of 264,192 bytes that every GPU loading this library holds until exit; it is sized for
+ * N <= MC_NOALLOC_MAX_N, a larger N is refused with MC_ENOSPACE (use mc_init + mc_energy there).  All calls on a
+ * device share that array: calls that may overlap on the GPU (different streams, or graphs replayed concurrently)
+ * race on it -- serialise them.  Nothing in the array has to be cleared between calls (every partial a call reads it
+ * has written first).  Agrees with mc_energy to rounding (<= 1e-9 relative; same decomposition, exact coordinate
+ * differences throughout). */
+#define MC_NOALLOC_MAX_N 131072
+int mc_energy_noalloc(int64_t N, const double* pos_dev /* [3][N] */, const double* charges_dev /* [N] */,
+                      double bjerrum_length, double* E_dev, void* stream);
+
 /* Adds the current configuration's ordered-pair distance counts into caller-owned device
  * accumulators: hist_dev [2][2][nbins] and n_centres_dev [2] (uint64).  Species index 0 if
  * q > 0 else 1.  Centres are ions with |x_i| <= centre_rmax (bulk only); partners

@@ -19,7 +19,7 @@ MC_OK, MC_EINVAL, MC_EOVERLAP, MC_EOUTSIDE, MC_ENOSPACE, MC_ECUDA, MC_ESTALL = 0
 _CODES = {-1: "MC_EINVAL", -2: "MC_EOVERLAP", -3: "MC_EOUTSIDE", -4: "MC_ENOSPACE", -5: "MC_ECUDA", -6: "MC_ESTALL"}
 
 EXPORTS = (
-    "mc_workspace_bytes", "mc_init", "mc_sweep", "mc_energy", "mc_energy_dev", "mc_pair_hist", "mc_sweep_host",
+    "mc_workspace_bytes", "mc_init", "mc_sweep", "mc_energy", "mc_energy_dev", "mc_energy_noalloc", "mc_pair_hist", "mc_sweep_host",
     "mc_sweep_timed", "mc_sweep_reduction",
     "mc_get_positions", "mc_set_positions", "mc_set_state", "mc_get_sweep_index", "mc_set_sweep_index", "mc_get_stats",
     "mc_get_trial_log", "mc_free", "mc_last_error", "mc_measure_fp64_peak", "mc_set_option", "mc_get_option",
@@ -58,6 +58,7 @@ def load_library() -> C.CDLL:
     lib.mc_sweep_reduction.argtypes = [vp, i64]
     lib.mc_energy.argtypes = [vp, C.POINTER(dbl)]
     lib.mc_energy_dev.argtypes = [vp, vp]
+    lib.mc_energy_noalloc.argtypes = [i64, vp, vp, dbl, vp, vp]
     lib.mc_sweep_timed.argtypes = [vp, i64, C.POINTER(dbl)]
     lib.mc_pair_hist.argtypes = [vp, dbl, C.c_int, dbl, vp, vp]
     lib.mc_sweep_host.argtypes = [vp, i64, vp, C.POINTER(dbl), vp, C.POINTER(mc_stats)]
@@ -114,6 +115,19 @@ def mc_measure_fp64_peak(millis: float = 50.0) -> float:
     _check(load_library().mc_measure_fp64_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), millis,
                                                C.byref(out)))
     return out.value
+
+
+def mc_energy_noalloc(pos: torch.Tensor, charges: torch.Tensor, bjerrum_length: float, out: torch.Tensor) -> torch.Tensor:
+    """From-scratch energy of the configuration ``pos`` ([3][N], CUDA float64) with ``charges`` ([N]) into ``out``
+    (CUDA float64, one element) on the current stream; allocates nothing (include/mcb200.h: mc_energy_noalloc)."""
+    for t in (pos, charges, out):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+    N = charges.numel()
+    assert tuple(pos.shape) == (3, N) and out.numel() >= 1
+    with torch.cuda.device(pos.device):
+        _check(load_library().mc_energy_noalloc(int(N), pos.data_ptr(), charges.data_ptr(), float(bjerrum_length),
+                                                out.data_ptr(), C.c_void_p(torch.cuda.current_stream().cuda_stream)))
+    return out
 
 
 class MCSystem:

@@ -8,6 +8,7 @@
 #include <cstddef>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -714,3 +715,140 @@ int mc_get_launch_count(mc_handle* h, uint64_t* n_host) {
 }
 
 }  // extern "C"
+
+// =============================================================================================
+// mc_energy_noalloc: the from-scratch energy (a5) for callers that cannot allocate device memory
+// (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  No handle,
+// no workspace: the per-CTA partial sums live in a file-scope __device__ array that every GPU loading
+// this library holds until exit.  Same decomposition and summation order as k_energy (aux_kernels.cuh)
+// with exact coordinate differences (reading G11), on the caller's raw arrays.
+// =============================================================================================
+namespace {
+
+// 1024 x 256 units of the upper triangle at N = MC_NOALLOC_MAX_N: sum_{rb < 128} (512 - 4 rb) = 33,024 partials
+constexpr int kNoAllocMaxUnits = 33024;
+static_assert(MC_NOALLOC_MAX_N % 1024 == 0, "the unit count below assumes whole row blocks");
+static_assert((MC_NOALLOC_MAX_N / 1024) * (MC_NOALLOC_MAX_N / 256) -
+                      4 * ((MC_NOALLOC_MAX_N / 1024 - 1) * (MC_NOALLOC_MAX_N / 1024) / 2) == kNoAllocMaxUnits, "unit count");
+static __device__ __align__(256) double g_noalloc_scratch[kNoAllocMaxUnits];   // 264,192 bytes per GPU
+
+// one unit = rows [rb 1024, rb 1024 + 1024) x columns [j0, j0 + 256), pairs j > i only; 4 rows per thread
+__global__ void __launch_bounds__(256, 2) k_energy_raw(const double* __restrict__ pos, const double* __restrict__ chg,
+                                                       int N, double* __restrict__ part) {
+    constexpr int kRows = 4, kBlock = 256 * kRows;
+    __shared__ double sx[kETile], sy[kETile], sz[kETile], sq[kETile];
+    __shared__ double red[8];
+    const int tid = threadIdx.x;
+    int unit = blockIdx.x, rb = 0;
+    for (;;) {
+        const int n = ((N - rb * kBlock) + kETile - 1) / kETile;
+        if (unit < n) break;
+        unit -= n;
+        ++rb;
+    }
+    const int j0 = rb * kBlock + unit * kETile;
+    const int cnt = min(kETile, N - j0);
+    double x[kRows], y[kRows], z[kRows], q[kRows], acc[kRows];
+#pragma unroll
+    for (int u = 0; u < kRows; ++u) {
+        const int i = rb * kBlock + u * 256 + tid;
+        const bool live = i < N;
+        x[u] = live ? pos[i] : 0.0; y[u] = live ? pos[(size_t)N + i] : 0.0; z[u] = live ? pos[2 * (size_t)N + i] : 0.0;
+        q[u] = live ? chg[i] : 0.0;
+        acc[u] = 0.0;
+    }
+    if (tid < cnt) {
+        sx[tid] = pos[j0 + tid]; sy[tid] = pos[(size_t)N + j0 + tid]; sz[tid] = pos[2 * (size_t)N + j0 + tid];
+        sq[tid] = chg[j0 + tid];
+    }
+    __syncthreads();
+    const bool diagonal = unit < kBlock / kETile;
+    if (!diagonal) {
+#pragma unroll 2
+        for (int j = 0; j < cnt; ++j) {
+            const double ax = sx[j], ay = sy[j], az = sz[j], aq = sq[j];
+#pragma unroll
+            for (int u = 0; u < kRows; ++u) {
+                const double r2 = dist2(__dadd_rn(x[u], -ax), __dadd_rn(y[u], -ay), __dadd_rn(z[u], -az));
+                acc[u] = __fma_rn(aq, rsqrt_fast(r2), acc[u]);
+            }
+        }
+    } else {
+        for (int j = 0; j < cnt; ++j) {
+            const double ax = sx[j], ay = sy[j], az = sz[j], aq = sq[j];
+#pragma unroll
+            for (int u = 0; u < kRows; ++u) {
+                const int i = rb * kBlock + u * 256 + tid;
+                if (j0 + j > i && i < N) {
+                    const double r2 = dist2(__dadd_rn(x[u], -ax), __dadd_rn(y[u], -ay), __dadd_rn(z[u], -az));
+                    acc[u] = __fma_rn(aq, rsqrt_fast(r2), acc[u]);
+                }
+            }
+        }
+    }
+    // off the diagonal a dead row (i >= N) sits at the origin with q = 0: its sum is finite unless an ion sits exactly
+    // there, so it is dropped explicitly rather than multiplied by zero
+    double v = 0.0;
+#pragma unroll
+    for (int u = 0; u < kRows; ++u) {
+        const int i = rb * kBlock + u * 256 + tid;
+        if (i < N) v = __dadd_rn(v, __dmul_rn(q[u], acc[u]));
+    }
+    v = warp_sum(v);
+    if ((tid & 31) == 0) red[tid >> 5] = v;
+    __syncthreads();
+    if (tid == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t = __dadd_rn(t, red[w]);
+        part[blockIdx.x] = t;
+    }
+}
+
+// *out = l_B * sum of the partials in index order (one warp)
+__global__ void __launch_bounds__(32) k_energy_raw_reduce(const double* __restrict__ part, int nparts, double lB, double* out) {
+    double acc = 0.0;
+    for (int k = threadIdx.x; k < nparts; k += 32) acc = __dadd_rn(acc, part[k]);
+    acc = warp_sum(acc);
+    if (threadIdx.x == 0) *out = __dmul_rn(lB, acc);
+}
+
+// device address of g_noalloc_scratch, looked up once per device with that device current (in host code the array's
+// name is a host-side stand-in, not a device address)
+constexpr int kNoAllocMaxDevices = 64;
+double* g_noalloc_ptr[kNoAllocMaxDevices] = {};
+std::mutex g_noalloc_mutex;
+
+}  // namespace
+
+extern "C" int mc_energy_noalloc(int64_t N, const double* pos_dev, const double* charges_dev, double bjerrum_length,
+                                 double* E_dev, void* stream) {
+    if (!pos_dev || !charges_dev || !E_dev) return fail(MC_EINVAL, "mc_energy_noalloc: null argument");
+    if (N < 1 || N > MC_NOALLOC_MAX_N)
+        return fail(MC_ENOSPACE, "mc_energy_noalloc: N = " + std::to_string(N) + " is outside 1.." +
+                                     std::to_string(MC_NOALLOC_MAX_N) + " (MC_NOALLOC_MAX_N: the size the static scratch "
+                                     "array is built for); use mc_init + mc_energy for larger systems");
+    if (!std::isfinite(bjerrum_length)) return fail(MC_EINVAL, "mc_energy_noalloc: bjerrum_length must be finite");
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(MC_EINVAL, "mc_energy_noalloc: device ordinal beyond 63");
+    double* scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        if (!g_noalloc_ptr[dev]) {
+            double* ptr = nullptr;
+            const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch);
+            if (e != cudaSuccess || !ptr)
+                return fail(MC_ECUDA, std::string("mc_energy_noalloc: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+            g_noalloc_ptr[dev] = ptr;
+        }
+        scratch = g_noalloc_ptr[dev];
+    }
+    const int units = energy_units((int)N, 4);
+    if (units > kNoAllocMaxUnits) return fail(MC_ENOSPACE, "mc_energy_noalloc: internal: unit count beyond the scratch array");
+    cudaStream_t st = (cudaStream_t)stream;
+    // every partial a call reads is written by that call first: nothing in the array has to start at zero
+    k_energy_raw<<<units, 256, 0, st>>>(pos_dev, charges_dev, (int)N, scratch);
+    k_energy_raw_reduce<<<1, 32, 0, st>>>(scratch, units, bjerrum_length, E_dev);
+    CUDA_TRY(cudaGetLastError());
+    return MC_OK;
+}
