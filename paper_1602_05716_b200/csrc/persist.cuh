@@ -3,7 +3,7 @@
 // grid = 2 CTAs per SM, all co-resident (cooperative launch).  CTA 0 is the chain: it resolves the
 // sweep's N decisions in ascending order.  Every other CTA is a worker that
 // pulls items from three queues (ticket counters in global memory):
-//   DIAG(c)  speculative corrections inside chunk c (as k_diag)                        (a2/a3)
+//   DIAG(c)  speculative corrections inside chunk c (in-chunk units)                        (a2/a3)
 //   FAR(c)   rows of chunk c x a slice of the columns outside chunks c-1 and c          (a2)
 //            DIAG and FAR of chunk c are released when the chain has finished chunk c-2
 //   FIX(c)   rows of chunk c x 16 columns of chunk c-1 at their final positions         (a2)
@@ -345,7 +345,7 @@ __device__ __forceinline__ int veto_from_min(int m, double h, double ov_tol) {
 }
 
 // FAR / FIX item: all rows of the chunk (ROWS per consumer thread) x virtual columns [v0, v1) of
-// the column space that starts at cbeg and skips [gap0, gap1).  Same inner loop as k_bulk; the
+// the column space that starts at cbeg and skips [gap0, gap1).  The
 // mbarrier ring persists across items (kring = stages used so far, identical in every thread).
 template <int ROWS, bool UNIFORM, int FORM>
 __device__ __forceinline__ void bulk_item(const Params& p, PShared& sh, unsigned& kring, int row0, int nrows,
