@@ -352,18 +352,21 @@ __global__ void __launch_bounds__(1024) k_centres_sorted(Params p, double centre
 // particles is skipped by the warp if its box is farther than the histogram's range from the warp's box (a CTA-wide
 // box of 256 centres lets 28 % of all pairs through at N = 65536, the warps' boxes 18 %: runs of a Z-order curve are
 // not compact enough for more.  A second variant -- hit masks per lane first, then each lane walking its own hits --
-// was 3x slower: the walk reads the staged columns at lane-dependent addresses).
+// was 3x slower: the walk reads the staged columns at lane-dependent addresses).  Each warp stages the sub-tiles it
+// needs in a slot of its own: staging a tile for the whole CTA cost two CTA barriers per tile at which the warps, which
+// mostly need different sub-tiles, waited for one another (0.72 -> 0.68 ms per mc_pair_hist at N = 65536).
 // The bin of a pair in range is floor(r / w) with r = sqrt(r^2) correctly rounded, as the oracle computes it; the
 // fast path takes r = r^2 * rsqrt(r^2) (a few ulp off) and falls back to the IEEE square root only where r / w is
 // within 1e-9 of an integer, so the counts stay bit-identical to the oracle's.
 __global__ void __launch_bounds__(256) k_hist(Params p, const int* list, const int* count, const double* bbox,
                                               double inv_w, int nbins, double cut2, unsigned long long* hist) {
     extern __shared__ unsigned shist[];  // [4][nbins]
-    __shared__ double2 sxy[256], szq[256];
-    const int tid = threadIdx.x;
+    __shared__ double2 sxy[8][kSubTile], szq[8][kSubTile];   // one staging slot per WARP: no CTA barrier in the tile loop
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int nc = *count;
     if ((int)blockIdx.x * 256 >= nc) return;
     for (int b = tid; b < 4 * nbins; b += 256) shist[b] = 0u;
+    __syncthreads();
     const int c = blockIdx.x * 256 + tid;
     const bool live = c < nc;
     const int i = live ? list[c] : -1;
@@ -383,10 +386,10 @@ __global__ void __launch_bounds__(256) k_hist(Params p, const int* list, const i
     const int ntile = (p.N + 255) / 256;
     const double margin = 1.0 + 1e-6;   // the cull is conservative: only sub-tiles clearly out of range are skipped
     for (int ct = blockIdx.y; ct < ntile; ct += gridDim.y) {
-        // which of the tile's 4 sub-tiles of 64 are in range of this warp's centres (the same in every lane)
-        unsigned inrange = 0u;
-#pragma unroll
+        const int j0 = ct * 256;
+        const int cnt = min(256, p.N - j0);
         for (int st = 0; st < 4; ++st) {
+            // is this sub-tile of 64 sorted particles in range of this warp's centres (the same in every lane)?
             const double* bb = bbox + ((size_t)ct * 4 + st) * 6;
             double d2 = 0.0;
 #pragma unroll
@@ -394,23 +397,23 @@ __global__ void __launch_bounds__(256) k_hist(Params p, const int* list, const i
                 const double gap = fmax(0.0, fmax(bb[2 * k] - wb[2 * k + 1], wb[2 * k] - bb[2 * k + 1]));
                 d2 += gap * gap;
             }
-            if (d2 <= cut2 * margin) inrange |= 1u << st;
-        }
-        // (also the barrier between the last tile's readers and this tile's staging, and after the zeroing of shist)
-        if (!__syncthreads_or((int)inrange)) continue;
-        const int j0 = ct * 256;
-        if (j0 + tid < p.N) { sxy[tid] = p.xy[j0 + tid]; szq[tid] = p.zq[j0 + tid]; }
-        __syncthreads();
-        const int cnt = min(256, p.N - j0);
-        if (!live) continue;
-        for (int st = 0; st < 4; ++st) {
-            if (!((inrange >> st) & 1u)) continue;
-            const int jend = min(cnt, (st + 1) * kSubTile);
+            if (!(d2 <= cut2 * margin) || st * kSubTile >= cnt) continue;
+            // the warp stages the sub-tile for itself (the other warps of the CTA mostly need other sub-tiles: a shared
+            // staging made them wait for one another at two CTA barriers per tile, 60 % of the kernel's stall cycles)
+            __syncwarp();
+#pragma unroll
+            for (int h = 0; h < kSubTile / 32; ++h) {
+                const int jj = st * kSubTile + h * 32 + lane;
+                if (jj < cnt) { sxy[warp][h * 32 + lane] = p.xy[j0 + jj]; szq[warp][h * 32 + lane] = p.zq[j0 + jj]; }
+            }
+            __syncwarp();
+            if (!live) continue;
+            const int jn = min(cnt - st * kSubTile, kSubTile);
 #pragma unroll 4
-            for (int j = st * kSubTile; j < jend; ++j) {
-                const double2 a = sxy[j], b = szq[j];
+            for (int j = 0; j < jn; ++j) {
+                const double2 a = sxy[warp][j], b = szq[warp][j];
                 const double r2 = dist2(__dadd_rn(xyi.x, -a.x), __dadd_rn(xyi.y, -a.y), __dadd_rn(zqi.x, -b.x));
-                if (r2 < cut2 && (j0 + j) != i) {
+                if (r2 < cut2 && (j0 + st * kSubTile + j) != i) {
                     const double t = __dmul_rn(__dmul_rn(r2, rsqrt_fast(r2)), inv_w);
                     double fb = floor(t);
                     const double frac = t - fb;
