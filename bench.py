@@ -286,16 +286,18 @@ def run_ours(args, w):
     e_run = [sysm.mc_get_stats()["E_running"]]
     pin_in.copy_(torch.from_numpy(sysm.positions))              # the chain's current state, with its running energy
 
+    pins = [pin_in, pin_out]
+
     def step_e2e():
         hist.zero_(); ncent.zero_()
         # H2D positions (+ the running energy that belongs to them: no from-scratch pass), sweep, D2H positions + stats
-        _, st = sysm.mc_sweep_host(1, pin_in, pin_out, E_running_in=e_run[0])
+        _, st = sysm.mc_sweep_host(1, pins[0], pins[1], E_running_in=e_run[0])
         e_run[0] = st["E_running"]
         sysm.mc_pair_hist(w.hist_bin_width, w.hist_nbins, w.hist_centre_rmax, hist, ncent)
         pin_hist.copy_(hist, non_blocking=True)
         pin_ncent.copy_(ncent, non_blocking=True)
         e = sysm.mc_energy()                                    # host scalar (synchronises)
-        pin_in.copy_(pin_out)                                   # the next step continues the chain
+        pins.reverse()                                          # the next step continues the chain: its input is this step's output buffer
         return st, e
 
     h2d = 3 * N * 8 + 8
